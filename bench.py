@@ -1,0 +1,413 @@
+#!/usr/bin/env python
+"""bench.py — drag-update throughput (cells/s, fp64) of the fused CUDA path, with its roofline and the CPU oracle.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--no-sweep] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (a1..a5) over one batch of synthetic input = ONE
+dg_drag_update launch over all cells of the workload.  Inputs are resident in HBM when the timed region starts;
+out of place (p_out != p_in) so every launch does identical work; the working set (GBs) is far larger than the 126 MB
+L2, so no L2 flush is needed between iterations.  Timing: CUDA events on the launching stream, barrier +
+synchronize on both sides, max over ranks.  --gpus N > 1 runs N independent replicas (the path does not
+shard, there is no collective on the data path); value = cells all ranks processed / max time.
+
+Prints ONE JSON line (rank 0).  Keys beyond the base contract: roofline, cpu_baseline, e2e, clocks, gpu_launches,
+peaks (the microbenchmarked denominators), sweep (the other BASELINE.json configs, device-timed the same way).
+--impl reference times the CPU oracle (oracle/) on the host cores on the same workload recipe.
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2509_25347_b200 import workloads as W  # noqa: E402
+
+METRIC = "drag-update cells/sec (fp64)"
+UNIT = "cells/s"
+# Table B.1 for the ALGORITHMIC flop count of SURVEY.md §8(d): rows (m, Pi_m, theta_m)
+TABLE_B1 = [(2, 1, 2.5809568e-8), (4, 2, 3.3971688e-4), (6, 3, 9.0656564e-3), (9, 4, 8.9577602e-2),
+            (12, 5, 2.9961589e-1), (16, 6, 7.8028743e-1), (20, 7, 1.4382526), (25, 8, 2.4285825), (30, 9, 3.5396663)]
+FP64_LANES_PER_SM = 64  # 4 sub-partitions x 16 fp64 FMA lanes (DESIGN.md §6 derives the ALU peak from this)
+
+
+def algorithmic_bytes_per_cell(N):
+    """read (2N+1) + 3(N+1) doubles, write 3(N+1) doubles = 8(8N+7) bytes."""
+    return 8 * (8 * N + 7)
+
+
+def algorithmic_flops(wl):
+    """F = [min_k (Pi_mk + s_k)] * 2 n^3 + 6 n^2 per cell, s_k = max(0, ceil(log2(||A||_1/theta_mk))),
+    summed over the workload's cells (the paper's own cost measure, B.11, times the dense product cost, plus the
+    apply).  Returns (total flops, mean products per cell)."""
+    n = wl.N + 1
+    eps = wl.rho_d / wl.rho_g[None, :]
+    a = wl.dt / wl.t_s
+    norm = 2.0 * torch.maximum((eps * a).sum(dim=0), a.max(dim=0).values)
+    best = None
+    for m, pi, theta in TABLE_B1:
+        s = torch.clamp(torch.ceil(torch.log2(norm / theta)), min=0.0)
+        cost = s + pi
+        best = cost if best is None else torch.minimum(best, cost)
+    products = float(best.sum().item())
+    return products * 2.0 * n ** 3 + 6.0 * n * n * wl.ncells, products / wl.ncells
+
+
+def executed_flops(N, s, m):
+    """Flops the thread-per-cell kernel actually issues (FMA = 2), from the per-cell (m, s) it reports: Horner steps in
+    the symmetric packed form, symmetric squarings with the conservation sums, and the apply."""
+    n = N + 1
+    tri = n * (n - 1) // 2
+    horner = n * n + (tri + n) * 2 + n          # row 0: n*n FMA; rows >= 1: 2 ops per packed entry; scale
+    square = tri * n + n * n                    # offdiag(X X) upper triangle + conservation sums
+    apply_ = 3 * (n * n + 2 * n)
+    sm = s.double()
+    mm = m.double()
+    fma = ((mm - 1).clamp(min=0) * horner + sm * square + apply_ + n * n).sum().item()
+    return 2.0 * fma
+
+
+class ClockSampler:
+    """SM clock, power and throttle reasons sampled through NVML every few ms WHILE the timed region runs
+    (start() right before the first timed launch, stop() right after the closing synchronize)."""
+    REASONS = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+               "hw_power_brake": 0x80}
+
+    def __init__(self, device_index, period_s=0.004):
+        self.period = period_s
+        self.rows = []
+        self.reasons = set()
+        self.handle = None
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                self.handle = pynvml.nvmlDeviceGetHandleByUUID(uuid if uuid.startswith("GPU-") else "GPU-" + uuid)
+            except Exception:
+                self.handle = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.handle = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.handle, nv.NVML_CLOCK_SM)
+                mw = nv.nvmlDeviceGetPowerUsage(self.handle)
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.handle)
+                self.rows.append((float(mhz), mw / 1000.0))
+                for name, bit in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.handle is None:
+            return
+        self._stop.clear()
+        self._thread = threading.Thread(target=self._loop, daemon=True)
+        self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join(timeout=2)
+            self._thread = None
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        sm = sorted(r[0] for r in self.rows)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_mhz_min": sm[0], "sm_max_mhz": self.max_mhz,
+                "power_w_max": max(r[1] for r in self.rows), "reasons": sorted(self.reasons), "samples": len(sm)}
+
+
+def aggregate_over_ranks(ms_local, cells_local):
+    """max over ranks of the timed region, sum over ranks of the cells processed (the only cross-rank step)."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms_local), int(cells_local)
+    dev = torch.device("cuda", torch.cuda.current_device()) if dist.get_backend() == "nccl" else torch.device("cpu")
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=dev)
+    c = torch.tensor([int(cells_local)], dtype=torch.int64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(c.item())
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.barrier()
+
+
+def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None):
+    """Returns (total ms over `steps` launches, list of per-launch ms)."""
+    for _ in range(warmup):
+        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    barrier()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.start()
+    ev[0].record()
+    for k in range(steps):
+        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+        ev[k + 1].record()
+    torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.stop()
+    barrier()
+    per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    return ev[0].elapsed_time(ev[steps]), per
+
+
+def measure_peaks(dg, device, sm_count, sm_max_mhz):
+    """The denominators MEASURED_PEAKS.json lacks: sustained DFMA / DMMA rates and an fp64 copy, one launch each timed
+    with CUDA events (best of 5 after a warm-up)."""
+    scratch = torch.empty(1 << 28, dtype=torch.float64, device=device)  # 2 GiB: copy 1 GiB -> 1 GiB
+    scratch.zero_()
+    out = {}
+    for name, kind, iters in (("dfma_tflops", 0, 20000), ("dmma_tflops", 1, 20000), ("dfma_dmma_mixed_tflops", 2, 5000),
+                              ("fp64_copy_gbs", 3, 1)):
+        best = None
+        for rep in range(6):
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            work = dg.dg_peak_kernel(kind, iters, scratch)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            if rep > 0:
+                best = ms if best is None else min(best, ms)
+        out[name] = work / (best * 1e-3) / (1e9 if kind == 3 else 1e12)
+    del scratch
+    out["fp64_nominal_tflops"] = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    return out
+
+
+def measured_peaks_file():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+def roofline_for(wl, ms_per_launch, alg_flops, peaks, hbm_gbs, hbm_src):
+    """The binding roofline of the fused kernel: whichever of (algorithmic bytes / HBM peak) and (algorithmic flops /
+    fp64 ALU peak) takes longer."""
+    nbytes = algorithmic_bytes_per_cell(wl.N) * wl.ncells
+    t_hbm = nbytes / (hbm_gbs * 1e9)
+    t_alu = alg_flops / (peaks["fp64_nominal_tflops"] * 1e12)
+    sec = ms_per_launch * 1e-3
+    if t_alu >= t_hbm:
+        ach = alg_flops / sec / 1e12
+        peak = peaks["fp64_nominal_tflops"]
+        return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                "peak_source": "nominal fp64 FMA peak = SMs x 64 lanes x 2 x clocks.max.sm (DESIGN.md §6); "
+                               "measured DFMA microbenchmark in peaks.dfma_tflops",
+                "frac_of_measured_dfma": ach / peaks["dfma_tflops"],
+                "hbm_frac": (nbytes / sec / 1e9) / hbm_gbs}
+    ach = nbytes / sec / 1e9
+    return {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs, "traffic": None,
+            "peak_source": hbm_src, "alu_frac": (alg_flops / sec / 1e12) / peaks["fp64_nominal_tflops"]}
+
+
+def cpu_oracle_sample(wl, budget_s=15.0):
+    """Times the oracle as it stands (all host threads) on a strided sample of the workload sized for ~budget_s."""
+    from oracle import dgo
+    threads = dgo.max_threads()
+
+    def run(nsample):
+        idx = W.sample_cells(wl.ncells, nsample)
+        rho_g, rho_d, t_s, p_in = wl.cells(idx)
+        t0 = time.perf_counter()
+        dgo.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+        return len(idx), time.perf_counter() - t0
+
+    dgo.lib()
+    nc, sec = run(min(wl.ncells, 2048))                     # calibration
+    rate = nc / max(sec, 1e-6)
+    nsample = int(min(wl.ncells, max(2048, rate * budget_s)))
+    nc, sec = run(nsample)
+    return {"value": nc / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{nc} cells strided over the {wl.ncells}-cell workload, {sec:.1f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same workload recipe, each step a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import dgo
+    wl = W.make_workload(args.config, ncells=min(W.CONFIG_CELLS[args.config], 1 << 20), N=args.N, device="cpu")
+    threads = dgo.max_threads()
+    dgo.lib()
+    idx = W.sample_cells(wl.ncells, 2048)
+    cells = wl.cells(idx)
+    t0 = time.perf_counter(); dgo.drag_update(cells[0], cells[1], cells[2], wl.dt, cells[3]); cal = time.perf_counter() - t0
+    total_budget = 120.0
+    per_step = total_budget / (args.steps + args.warmup)
+    nsample = int(min(wl.ncells, max(1024, len(idx) / max(cal, 1e-6) * per_step)))
+    idx = W.sample_cells(wl.ncells, nsample)
+    cells = wl.cells(idx)
+    for _ in range(args.warmup):
+        dgo.drag_update(cells[0], cells[1], cells[2], wl.dt, cells[3])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        dgo.drag_update(cells[0], cells[1], cells[2], wl.dt, cells[3])
+    sec = time.perf_counter() - t0
+    value = len(idx) * args.steps / sec
+    sample = f"{len(idx)} cells per step strided over the first {wl.ncells} cells of the recipe"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
+        "config": {"workload": wl.name.split("_")[0] + f"_N{wl.N}", "recipe": f"BASELINE.json configs[{args.config - 1}]",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, want_exec=True, sampler=None):
+    p_out = torch.empty_like(wl.p_in)
+    total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
+    alg_flops, products = algorithmic_flops(wl)
+    ms_launch = sum(per) / len(per)
+    roof = roofline_for(wl, ms_launch, alg_flops, peaks, hbm_gbs, hbm_src)
+    res = {"workload": wl.name, "N": wl.N, "ncells": wl.ncells, "ms_per_step": total_ms / steps,
+           "ms_per_launch_min": min(per), "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
+           "algorithmic_flops_per_cell": alg_flops / wl.ncells, "algorithmic_products_per_cell": products,
+           "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N), "roofline": roof,
+           "variant": dg.dg_variant_name(wl.N)}
+    if want_exec:
+        _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+        ex = executed_flops(wl.N, s, m)
+        res["executed_flops_per_cell"] = ex / wl.ncells
+        res["executed_tflops"] = ex / (ms_launch * 1e-3) / 1e12
+        res["mean_s"] = float(s.double().mean().item()); res["mean_m"] = float(m.double().mean().item())
+        res["max_s"] = int(s.max().item())
+    del p_out
+    return res, total_ms
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[config-1]; 5 = sweep point (give --N)")
+    ap.add_argument("--N", type=int, default=None)
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.config == 5 and args.N is None:
+        args.N = 16
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2509_25347_b200 import binding as dg  # raises if libdg.so is missing
+
+    props = torch.cuda.get_device_properties(device)
+    mp_file, hbm_src = measured_peaks_file()
+    hbm_gbs = float(mp_file["hbm_gbs"])
+    sm_max_mhz = float(mp_file.get("sm_max_mhz", 1965.0))
+    peaks = measure_peaks(dg, device, props.multi_processor_count, sm_max_mhz)
+
+    # replicas: every rank runs the same recipe with its own seed
+    wl = W.make_workload(args.config, N=args.N, device=device, seed=rank)
+    clk = ClockSampler(local_rank)
+    res, total_ms = bench_one(dg, wl, args.steps, args.warmup, peaks, hbm_gbs, hbm_src, sampler=clk)
+    clocks = clk.summary()
+    ms_max, cells_all = aggregate_over_ranks(total_ms, wl.ncells * args.steps)
+    value = cells_all / (ms_max * 1e-3)
+
+    # end to end through the host-buffer C-ABI call: pinned host tensors -> H2D -> kernel -> D2H, every step
+    e2e = None
+    if not args.no_e2e:
+        n = wl.N + 1
+        host = [t.cpu().pin_memory() for t in (wl.rho_g, wl.rho_d, wl.t_s, wl.p_in)]
+        h_out = torch.empty_like(host[3]).pin_memory()
+        e2e_steps = max(1, min(args.steps, 3))
+        dg.dg_drag_update_host(host[0], host[1], host[2], wl.dt, host[3], p_out=h_out)  # warm-up (allocates staging)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            dg.dg_drag_update_host(host[0], host[1], host[2], wl.dt, host[3], p_out=h_out)
+        sec = time.perf_counter() - t0
+        barrier()
+        ms_e2e, cells_e2e = aggregate_over_ranks(sec * 1e3, wl.ncells * e2e_steps)
+        e2e = {"value": cells_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": 8 * (1 + 2 * wl.N + 3 * n) * wl.ncells, "d2h_bytes_per_step": 8 * 3 * n * wl.ncells,
+               "steps": e2e_steps, "api": "dg_drag_update_host (pinned host buffers, chunked, 3 streams)"}
+        dg.dg_host_release()
+        del host, h_out
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_oracle_sample(wl)
+
+    sweep = []
+    if rank == 0 and world == 1 and not args.no_sweep:
+        del wl
+        torch.cuda.empty_cache()
+        points = [(c, None) for c in (2, 3, 4) if c != args.config] + [(5, N) for N in W.SWEEP_N]
+        for cfg, N in points:
+            w2 = W.make_workload(cfg, N=N, device=device)
+            r2, _ = bench_one(dg, w2, max(3, min(args.steps, 5)), 3, peaks, hbm_gbs, hbm_src)
+            sweep.append(r2)
+            del w2
+            torch.cuda.empty_cache()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": res["workload"], "recipe": f"BASELINE.json configs[{args.config - 1}]",
+                       "N": res["N"], "ncells_per_gpu": res["ncells"], "parallelism": "replicas" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (no flush)", "variant": res["variant"],
+                       "paper_context": "A100/Dyablo N=8: 9.7e-9 s/cell = 1.03e8 cells/s (PAPER.md:341); other machine"},
+            "roofline": res["roofline"], "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+            "gpu_launches": args.steps * dg.dg_launches_per_update(res["N"], res["ncells"]),
+            "peaks": dict(peaks, hbm_gbs=hbm_gbs, hbm_source=hbm_src, gpu=props.name, sms=props.multi_processor_count),
+            "detail": {k: v for k, v in res.items() if k not in ("roofline",)},
+            "sweep": sweep,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,123 @@
+/*
+ * dg.h — C ABI of libdg: the per-cell exponential drag update for a gas + N dust fluids (arXiv 2509.25347) on
+ * NVIDIA B200 (sm_100a).  PAPER.md below is the extracted text of the paper; citations are PAPER.md:<line>.
+ *
+ * What the library computes, per cell and independently of every other cell (footnote 1):
+ *     p_out[comp] = exp(dt * Omega) * p_in[comp],   comp = x, y, z                    (Eq. 18)
+ * where Omega is the (N+1) x (N+1) drag matrix of Eq. 17 built from that cell's
+ *     eps_i = rho_d,i / rho_g (Eq. 14)   and   alpha_i = 1 / t_s,i (Eq. 15),
+ * and exp() is evaluated by Taylor-based scaling and squaring (Sect. 2.3; Alg. 6):
+ * a norm-based choice of (m, s) from the thresholds of Table B.1, the degree-m Taylor polynomial
+ * of A / 2^s (Eq. 19), then s squarings (Eq. 23-24).  Species index 0 is the gas.
+ *
+ * ---------------------------------------------------------------------------------------------------------------
+ * Layouts.  Structure of arrays, fp64, cell index c fastest (0 <= c < ncells), n = N + 1, 1 <= N <= DG_NMAX:
+ *     rho_g [ncells]             gas density                                  > 0
+ *     rho_d [N][ncells]          dust densities                               >= 0
+ *     t_s   [N][ncells]          stopping times                               > 0
+ *     p     [3][n][ncells]       momenta (component, species, cell)           Eq. 13
+ *     A, E  [n*n][ncells]        matrices, element r*n + col; row r = destination species, col = source species
+ *     s_out [ncells]             int32, the scaling exponent s chosen in each cell
+ * "Device pointer" = memory the GPU can address (cudaMalloc / a torch CUDA tensor's data_ptr()).
+ * "Host pointer"   = ordinary host memory; page-locked (pinned) memory makes the copies asynchronous.
+ *
+ * Ownership.  The library owns no caller-visible memory and keeps no global state that affects results.  All
+ * buffers are caller-allocated and caller-freed.  The dg_* device entry points allocate nothing and use no
+ * workspace.  dg_drag_update_host keeps a private device staging area that dg_host_release() frees.
+ *
+ * Streams and asynchrony.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ * entry points only enqueue work and return; they never synchronise.  They are re-entrant and may be called
+ * concurrently on different streams.  Results are bitwise reproducible for a fixed build and GPU.
+ *
+ * Errors.  Every entry point returns a dg_status; nothing throws or aborts across the ABI:
+ *     DG_ENULL   a required pointer is NULL (checked only when ncells > 0)
+ *     DG_ERANGE  N outside [1, DG_NMAX] or ncells < 0
+ *     DG_EALIGN  a pointer is not 8-byte aligned
+ *     DG_EINVAL  dt negative or not finite, or another scalar argument outside its documented range
+ *     DG_ECUDA   the CUDA runtime reported an error (cudaGetLastError after the launch, or a failed copy/alloc);
+ *                dg_last_cuda_error() returns its text
+ * ncells == 0 is DG_OK and a no-op.
+ *
+ * Pre-conditions that are NOT checked on the device (PAPER.md is silent; they are what Eq. 14-15 need):
+ * rho_g > 0, rho_d >= 0, t_s > 0, everything finite, rho_d / rho_g <= 1e200.  A cell that violates them yields
+ * non-finite or meaningless output in that cell only.  dt = 0 returns p_out == p_in bit for bit.
+ * rho_d,i = 0 is allowed: species i then receives nothing from the gas (column-0 entry i of Eq. 17 is zero).
+ */
+#ifndef DG_H
+#define DG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DG_NMAX 16
+#define DG_VERSION 100 /* 0.1.0 */
+
+typedef enum { DG_OK = 0, DG_EINVAL = 1, DG_ENULL = 2, DG_EALIGN = 3, DG_ERANGE = 4, DG_ECUDA = 5 } dg_status;
+
+/* ---- stage a1: assemble A = dt * Omega  (Eq. 14, 15, 17) ---------------------------------
+ * in : rho_g, rho_d, t_s (device), dt.   out: A [n*n][ncells] (device), dense, including the structural zeros.
+ * Off-diagonals: A[0][i] = dt/t_s,i, A[i][0] = (rho_d,i/rho_g) * dt/t_s,i.  Each diagonal entry is minus the sum
+ * of the off-diagonal entries of its column (columns of Eq. 17 sum to zero: total momentum). */
+dg_status dg_drag_matrix_build(const double* rho_g, const double* rho_d, const double* t_s, double dt, int N,
+                               long long ncells, double* A, void* stream);
+
+/* ---- stages a2-a4: E = exp(A) by scaling and squaring  (Sect. 2.3, Alg. 6, Table B.1) -----------------------
+ * in : A [n*n][ncells] (device) — MUST be a drag matrix of Eq. 17 as dg_drag_matrix_build writes it: only the
+ *      off-diagonal entries of row 0 and column 0 are read (A[0][i] >= 0, A[i][0] >= 0); the stored diagonal and
+ *      the structural zeros are ignored and the diagonal is re-derived from the zero-column-sum property.  This is
+ *      not a general-purpose expm.
+ * out: E [n*n][ncells] (device), may alias A.  Entries are in [0,1] and every column sums to 1 to rounding.
+ *      s_out (device, int32 [ncells], nullable): the scaling exponent chosen per cell (number of squarings). */
+dg_status dg_expm_scale_square(const double* A, int N, long long ncells, double* E, int* s_out, void* stream);
+
+/* ---- stage a5: p_out[comp] = E * p_in[comp] for the three components  (Eq. 18) ----------------
+ * in : E [n*n][ncells], p_in [3][n][ncells] (device).   out: p_out [3][n][ncells] (device), may alias p_in. */
+dg_status dg_drag_apply(const double* E, const double* p_in, int N, long long ncells, double* p_out, void* stream);
+
+/* ---- fused a1..a5 in one kernel; no matrix ever reaches HBM.  This is the timed path. -----------------------
+ * in : rho_g, rho_d, t_s, p_in (device), dt.   out: p_out (device), may alias p_in.
+ * HBM traffic per cell: 8*(8N+7) bytes. */
+dg_status dg_drag_update(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
+                         int N, long long ncells, double* p_out, void* stream);
+
+/* Same as dg_drag_update and additionally writes s_out[c] (device int32 [ncells], nullable) and m_out[c]
+ * (device int32 [ncells], nullable): the scaling exponent and Taylor degree chosen in each cell. */
+dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                            const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
+                            void* stream);
+
+/* ---- the same update on HOST buffers (end-to-end path) -------------------------------------------------------
+ * All array arguments are HOST pointers in the layouts above.  The call cuts the cells into chunks of
+ * `chunk_cells` (0 = library default), copies each chunk's inputs to a private device staging area, runs the
+ * fused kernel and copies the result back, overlapping the three on internal streams; it returns after the last
+ * copy has completed (it synchronises).  Page-locked host buffers make the copies truly asynchronous; pageable
+ * buffers work but serialise.  p_out may alias p_in.  `device` is the CUDA device ordinal (-1 = current). */
+dg_status dg_drag_update_host(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                              const double* p_in, int N, long long ncells, double* p_out, long long chunk_cells,
+                              int device);
+/* Frees the staging area and streams of dg_drag_update_host (all devices).  Safe to call at any time. */
+dg_status dg_host_release(void);
+
+/* ---- measurement helpers (used by bench.py; not on the data path) --------------------------------------------
+ * dg_peak_kernel enqueues ONE launch of a microbenchmark kernel on `stream` and returns in *work the number of
+ * flops (kinds 0-2; FMA = 2) or bytes (kind 3) that launch performs; the caller times it with events.
+ *   kind 0: independent fp64 FMA chains (DFMA), all SMs        kind 1: fp64 tensor-core tiles (DMMA m8n8k4)
+ *   kind 2: DFMA and DMMA interleaved in the same warps        kind 3: fp64 SoA copy (read + write bytes)
+ * scratch: device buffer of at least scratch_bytes bytes (>= 1 MiB; kind 3 copies its first half to its second).
+ * iters: loop trip count per thread (kinds 0-2). */
+dg_status dg_peak_kernel(int kind, int iters, double* scratch, long long scratch_bytes, double* work, void* stream);
+
+/* Number of kernels the last device entry point launched for these arguments (the launch plan; 0 if ncells == 0). */
+int dg_launches_per_update(int N, long long ncells);
+/* Human-readable description of the kernel variant dg_drag_update uses for N (static storage). */
+const char* dg_variant_name(int N);
+
+const char* dg_status_string(dg_status st); /* static storage */
+const char* dg_last_cuda_error(void);       /* static storage; "" if none */
+int dg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DG_H */

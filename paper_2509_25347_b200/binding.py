@@ -1,0 +1,199 @@
+"""Thin ctypes binding over libdg.so (include/dg.h): argument marshalling only — every step of the path runs in
+the CUDA kernels of the library.  Function names are those of the C ABI.
+
+Device entry points take torch CUDA float64 tensors in the layouts of include/dg.h and enqueue on torch's current
+stream; PyTorch is used for device memory and streams only.  There is no CPU fallback: if libdg.so is missing or
+cannot be loaded, importing this module raises.
+"""
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libdg.so")
+
+DG_NMAX = 16
+DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
+
+EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
+           "dg_drag_update_host", "dg_host_release", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
+           "dg_status_string", "dg_last_cuda_error", "dg_version")
+
+
+class DgError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        msg = _lib.dg_status_string(self.status).decode()
+        if self.status == DG_ECUDA:
+            msg += " — " + _lib.dg_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg}")
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2509_25347_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dbl, ll, i32 = C.c_void_p, C.c_double, C.c_longlong, C.c_int
+    lib.dg_drag_matrix_build.argtypes = [vp, vp, vp, dbl, i32, ll, vp, vp]
+    lib.dg_expm_scale_square.argtypes = [vp, i32, ll, vp, vp, vp]
+    lib.dg_drag_apply.argtypes = [vp, vp, i32, ll, vp, vp]
+    lib.dg_drag_update.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
+    lib.dg_drag_update_ex.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp, vp, vp]
+    lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
+    lib.dg_host_release.argtypes = []
+    lib.dg_peak_kernel.argtypes = [i32, i32, vp, ll, C.POINTER(dbl), vp]
+    lib.dg_launches_per_update.argtypes = [i32, ll]
+    lib.dg_variant_name.argtypes = [i32]
+    lib.dg_variant_name.restype = C.c_char_p
+    lib.dg_status_string.argtypes = [i32]
+    lib.dg_status_string.restype = C.c_char_p
+    lib.dg_last_cuda_error.argtypes = []
+    lib.dg_last_cuda_error.restype = C.c_char_p
+    lib.dg_version.argtypes = []
+    for name in EXPORTS:
+        fn = getattr(lib, name)
+        if fn.restype is C.c_int and name not in ("dg_launches_per_update", "dg_version"):
+            fn.restype = C.c_int
+    return lib
+
+
+_lib = _load()
+
+
+def raw():
+    """The ctypes library handle (tests call it with deliberately bad arguments)."""
+    return _lib
+
+
+def _check(st, where):
+    if st != DG_OK:
+        raise DgError(st, where)
+
+
+def _dev(t, name, shape=None, dtype=torch.float64):
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name}: expected a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous {dtype} tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def _stream():
+    return torch.cuda.current_stream().cuda_stream
+
+
+def dg_drag_matrix_build(rho_g, rho_d, t_s, dt, A=None):
+    """Stage a1.  Returns A [n*n, ncells] = dt*Omega (Eq. 17)."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if A is None:
+        A = torch.empty((n * n, ncells), dtype=torch.float64, device=rho_g.device)
+    st = _lib.dg_drag_matrix_build(_dev(rho_g, "rho_g", (ncells,)), _dev(rho_d, "rho_d", (N, ncells)),
+                                   _dev(t_s, "t_s", (N, ncells)), float(dt), N, ncells,
+                                   _dev(A, "A", (n * n, ncells)), _stream())
+    _check(st, "dg_drag_matrix_build")
+    return A
+
+
+def dg_expm_scale_square(A, N, E=None, want_s=False):
+    """Stages a2-a4.  Returns E [n*n, ncells] = exp(A) (and the per-cell scaling exponent s if want_s)."""
+    n = N + 1
+    ncells = A.shape[1]
+    if E is None:
+        E = torch.empty_like(A)
+    s = torch.empty(ncells, dtype=torch.int32, device=A.device) if want_s else None
+    st = _lib.dg_expm_scale_square(_dev(A, "A", (n * n, ncells)), N, ncells, _dev(E, "E", (n * n, ncells)),
+                                   _dev(s, "s_out", (ncells,), torch.int32) if want_s else None, _stream())
+    _check(st, "dg_expm_scale_square")
+    return (E, s) if want_s else E
+
+
+def dg_drag_apply(E, p_in, N, p_out=None):
+    """Stage a5.  Returns p_out [3, n, ncells] = E p_in."""
+    n = N + 1
+    ncells = E.shape[1]
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    st = _lib.dg_drag_apply(_dev(E, "E", (n * n, ncells)), _dev(p_in, "p_in", (3, n, ncells)), N, ncells,
+                            _dev(p_out, "p_out", (3, n, ncells)), _stream())
+    _check(st, "dg_drag_apply")
+    return p_out
+
+
+def dg_drag_update(rho_g, rho_d, t_s, dt, p_in, p_out=None):
+    """Fused a1..a5 (the timed path).  Returns p_out [3, n, ncells]."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    st = _lib.dg_drag_update(_dev(rho_g, "rho_g", (ncells,)), _dev(rho_d, "rho_d", (N, ncells)),
+                             _dev(t_s, "t_s", (N, ncells)), float(dt), _dev(p_in, "p_in", (3, n, ncells)), N, ncells,
+                             _dev(p_out, "p_out", (3, n, ncells)), _stream())
+    _check(st, "dg_drag_update")
+    return p_out
+
+
+def dg_drag_update_ex(rho_g, rho_d, t_s, dt, p_in, p_out=None):
+    """Fused update that also returns the per-cell (s, m) choices: (p_out, s int32[ncells], m int32[ncells])."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    s = torch.empty(ncells, dtype=torch.int32, device=rho_g.device)
+    m = torch.empty(ncells, dtype=torch.int32, device=rho_g.device)
+    st = _lib.dg_drag_update_ex(_dev(rho_g, "rho_g", (ncells,)), _dev(rho_d, "rho_d", (N, ncells)),
+                                _dev(t_s, "t_s", (N, ncells)), float(dt), _dev(p_in, "p_in", (3, n, ncells)), N,
+                                ncells, _dev(p_out, "p_out", (3, n, ncells)), _dev(s, "s", (ncells,), torch.int32),
+                                _dev(m, "m", (ncells,), torch.int32), _stream())
+    _check(st, "dg_drag_update_ex")
+    return p_out, s, m
+
+
+def _host(t, name, shape):
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous float64 CPU tensor")
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def dg_drag_update_host(rho_g, rho_d, t_s, dt, p_in, p_out=None, chunk_cells=0, device=-1):
+    """The fused update on HOST tensors (pinned memory makes the copies asynchronous).  Synchronous."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    st = _lib.dg_drag_update_host(_host(rho_g, "rho_g", (ncells,)), _host(rho_d, "rho_d", (N, ncells)),
+                                  _host(t_s, "t_s", (N, ncells)), float(dt), _host(p_in, "p_in", (3, n, ncells)), N,
+                                  ncells, _host(p_out, "p_out", (3, n, ncells)), int(chunk_cells), int(device))
+    _check(st, "dg_drag_update_host")
+    return p_out
+
+
+def dg_host_release():
+    _check(_lib.dg_host_release(), "dg_host_release")
+
+
+def dg_peak_kernel(kind, iters, scratch):
+    """Enqueues one microbenchmark launch on the current stream; returns the flops (kinds 0-2) or bytes (kind 3)."""
+    work = C.c_double(0.0)
+    st = _lib.dg_peak_kernel(int(kind), int(iters), _dev(scratch, "scratch"), scratch.numel() * 8, C.byref(work),
+                             _stream())
+    _check(st, "dg_peak_kernel")
+    return work.value
+
+
+def dg_launches_per_update(N, ncells):
+    return int(_lib.dg_launches_per_update(int(N), int(ncells)))
+
+
+def dg_variant_name(N):
+    return _lib.dg_variant_name(int(N)).decode()
+
+
+def dg_version():
+    return int(_lib.dg_version())

@@ -1,0 +1,142 @@
+// dg_api.cu — the C ABI of include/dg.h: argument validation and dispatch on N.  No arithmetic here.
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+
+#include "../../include/dg.h"
+#include "dg_internal.h"
+
+namespace dg {
+
+static const Launchers* const kTable[DG_NMAX + 1] = {
+    nullptr,        &launchers_N1,  &launchers_N2,  &launchers_N3,  &launchers_N4,  &launchers_N5,
+    &launchers_N6,  &launchers_N7,  &launchers_N8,  &launchers_N9,  &launchers_N10, &launchers_N11,
+    &launchers_N12, &launchers_N13, &launchers_N14, &launchers_N15, &launchers_N16};
+
+static thread_local char g_cuda_err[256] = "";
+
+dg_status cuda_status(cudaError_t e) {
+    if (e == cudaSuccess) return DG_OK;
+    snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return DG_ECUDA;
+}
+
+static inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 7u) != 0; }
+
+// Common checks.  Returns DG_OK with *noop = true when there is nothing to do.
+static dg_status check_common(int N, long long ncells, bool* noop) {
+    *noop = false;
+    if (N < 1 || N > DG_NMAX || ncells < 0) return DG_ERANGE;
+    if (ncells == 0) *noop = true;
+    return DG_OK;
+}
+
+const Launchers* launchers_for(int N) { return (N >= 1 && N <= DG_NMAX) ? kTable[N] : nullptr; }
+
+}  // namespace dg
+
+using namespace dg;
+
+#define DG_CHECK_PTR(p)                  \
+    do {                                 \
+        if ((p) == nullptr) return DG_ENULL; \
+        if (misaligned(p)) return DG_EALIGN; \
+    } while (0)
+#define DG_CHECK_OPT_PTR(p)                            \
+    do {                                               \
+        if ((p) != nullptr && (reinterpret_cast<uintptr_t>(p) & 3u)) return DG_EALIGN; \
+    } while (0)
+
+extern "C" {
+
+dg_status dg_drag_matrix_build(const double* rho_g, const double* rho_d, const double* t_s, double dt, int N,
+                               long long ncells, double* A, void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
+    if (noop) return DG_OK;
+    DG_CHECK_PTR(rho_g);
+    DG_CHECK_PTR(rho_d);
+    DG_CHECK_PTR(t_s);
+    DG_CHECK_PTR(A);
+    BuildArgs a{rho_g, rho_d, t_s, dt, ncells, A};
+    return cuda_status(kTable[N]->build(a, static_cast<cudaStream_t>(stream)));
+}
+
+dg_status dg_expm_scale_square(const double* A, int N, long long ncells, double* E, int* s_out, void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (noop) return DG_OK;
+    DG_CHECK_PTR(A);
+    DG_CHECK_PTR(E);
+    DG_CHECK_OPT_PTR(s_out);
+    ExpmArgs a{A, ncells, E, s_out};
+    return cuda_status(kTable[N]->expm(a, static_cast<cudaStream_t>(stream)));
+}
+
+dg_status dg_drag_apply(const double* E, const double* p_in, int N, long long ncells, double* p_out, void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (noop) return DG_OK;
+    DG_CHECK_PTR(E);
+    DG_CHECK_PTR(p_in);
+    DG_CHECK_PTR(p_out);
+    ApplyArgs a{E, p_in, ncells, p_out};
+    return cuda_status(kTable[N]->apply(a, static_cast<cudaStream_t>(stream)));
+}
+
+dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                            const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
+                            void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
+    if (noop) return DG_OK;
+    DG_CHECK_PTR(rho_g);
+    DG_CHECK_PTR(rho_d);
+    DG_CHECK_PTR(t_s);
+    DG_CHECK_PTR(p_in);
+    DG_CHECK_PTR(p_out);
+    DG_CHECK_OPT_PTR(s_out);
+    DG_CHECK_OPT_PTR(m_out);
+    UpdateArgs a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, s_out, m_out};
+    return cuda_status(kTable[N]->update(a, static_cast<cudaStream_t>(stream)));
+}
+
+dg_status dg_drag_update(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
+                         int N, long long ncells, double* p_out, void* stream) {
+    return dg_drag_update_ex(rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, nullptr, nullptr, stream);
+}
+
+int dg_launches_per_update(int N, long long ncells) {
+    if (N < 1 || N > DG_NMAX || ncells <= 0) return 0;
+    return 1;
+}
+
+const char* dg_variant_name(int N) {
+    if (N < 1 || N > DG_NMAX) return "";
+    return kTable[N]->variant;
+}
+
+const char* dg_status_string(dg_status st) {
+    switch (st) {
+        case DG_OK: return "DG_OK";
+        case DG_EINVAL: return "DG_EINVAL: scalar argument out of range (dt negative or not finite)";
+        case DG_ENULL: return "DG_ENULL: required pointer is NULL";
+        case DG_EALIGN: return "DG_EALIGN: pointer is not 8-byte aligned";
+        case DG_ERANGE: return "DG_ERANGE: N outside [1, 16] or ncells < 0";
+        case DG_ECUDA: return "DG_ECUDA: CUDA runtime error (see dg_last_cuda_error)";
+    }
+    return "unknown dg_status";
+}
+
+const char* dg_last_cuda_error(void) { return g_cuda_err; }
+
+int dg_version(void) { return DG_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,67 @@
+// dg_internal.h — declarations shared by the translation units of libdg (not installed, not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace dg {
+
+struct UpdateArgs {  // dg_drag_update / dg_drag_update_ex
+    const double* rho_g;
+    const double* rho_d;
+    const double* t_s;
+    double dt;
+    const double* p_in;
+    long long ncells;
+    double* p_out;
+    int* s_out;
+    int* m_out;
+};
+struct BuildArgs {  // dg_drag_matrix_build
+    const double* rho_g;
+    const double* rho_d;
+    const double* t_s;
+    double dt;
+    long long ncells;
+    double* A;
+};
+struct ExpmArgs {  // dg_expm_scale_square
+    const double* A;
+    long long ncells;
+    double* E;
+    int* s_out;
+};
+struct ApplyArgs {  // dg_drag_apply
+    const double* E;
+    const double* p_in;
+    long long ncells;
+    double* p_out;
+};
+
+// One set of launchers per N (a translation unit each, compiled from dg_kernels.cu with -DDG_N=<N>).
+struct Launchers {
+    cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    cudaError_t (*build)(const BuildArgs&, cudaStream_t);
+    cudaError_t (*expm)(const ExpmArgs&, cudaStream_t);
+    cudaError_t (*apply)(const ApplyArgs&, cudaStream_t);
+    const char* variant;
+};
+
+#define DG_DECL_LAUNCHERS(NN) extern const Launchers launchers_N##NN;
+DG_DECL_LAUNCHERS(1)
+DG_DECL_LAUNCHERS(2)
+DG_DECL_LAUNCHERS(3)
+DG_DECL_LAUNCHERS(4)
+DG_DECL_LAUNCHERS(5)
+DG_DECL_LAUNCHERS(6)
+DG_DECL_LAUNCHERS(7)
+DG_DECL_LAUNCHERS(8)
+DG_DECL_LAUNCHERS(9)
+DG_DECL_LAUNCHERS(10)
+DG_DECL_LAUNCHERS(11)
+DG_DECL_LAUNCHERS(12)
+DG_DECL_LAUNCHERS(13)
+DG_DECL_LAUNCHERS(14)
+DG_DECL_LAUNCHERS(15)
+DG_DECL_LAUNCHERS(16)
+#undef DG_DECL_LAUNCHERS
+
+}  // namespace dg

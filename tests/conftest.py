@@ -17,3 +17,21 @@ def oracle():
     from oracle import dgo
     dgo.lib()
     return dgo
+
+
+@pytest.fixture(scope="session")
+def dg():
+    """The Python binding over libdg.so.  Builds the library if it is missing (nvcc cross-compiles without a GPU);
+    a failure to build or load is an error, never a skip: there is no fallback path."""
+    from paper_2509_25347_b200 import build
+    build.build()
+    from paper_2509_25347_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="session")
+def cuda(dg):
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    torch.cuda.set_device(0)
+    return torch.device("cuda:0")

@@ -1,0 +1,223 @@
+"""Parity of the CUDA path (through the C ABI of include/dg.h) with the CPU oracle, element by element, on the
+same seeded inputs (-m gpu).
+
+Tolerances are BASELINE.json's (reading R13), written here:
+  parity       per cell  max_{k,comp} |p_gpu - p_oracle|  <=  1e-12 * max_{k,comp} |p_in|
+  conservation per cell and component  |sum_k p_out - sum_k p_in|  <=  1e-13 * sum_k |p_in|
+Differences are formed in long double from the GPU's fp64 output and the oracle's long-double output.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2509_25347_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+PARITY_TOL = 1e-12
+CONS_TOL = 1e-13
+LD = np.longdouble
+
+
+def run_and_compare(dg, oracle, wl, idx=None, check_s=True):
+    """Runs the fused kernel on the whole workload and compares the cells `idx` (default: all) with the oracle."""
+    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    torch.cuda.synchronize()
+    if idx is None:
+        idx = torch.arange(wl.ncells)
+    idx_d = idx.to(wl.rho_g.device)
+    rho_g, rho_d, t_s, p_in = wl.cells(idx)
+    got = out[:, :, idx_d].cpu().numpy()
+    ref = oracle.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+    err = oracle.parity_error(got, ref, p_in)
+    cons = oracle.conservation_error(got, p_in)
+    assert np.isfinite(got).all()
+    assert float(err.max()) <= PARITY_TOL, f"{wl.name}: parity {float(err.max()):.3e} at cell {int(idx[int(err.argmax())])}"
+    assert float(cons.max()) <= CONS_TOL, f"{wl.name}: conservation {float(cons.max()):.3e}"
+    sv = s[idx_d].cpu().numpy(); mv = m[idx_d].cpu().numpy()
+    if check_s:
+        # the (m, s) choice must satisfy Theorem 1's premise: ||A||_1 / 2^s <= theta_m (Table B.1)
+        theta = {2: 2.5809568e-8, 4: 3.3971688e-4, 6: 9.0656564e-3, 9: 8.9577602e-2, 12: 2.9961589e-1, 16: 7.8028743e-1,
+                 20: 1.4382526, 25: 2.4285825, 30: 3.5396663}
+        eps = rho_d / rho_g[None, :]
+        a = wl.dt / t_s
+        norm = 2.0 * np.maximum((eps * a).sum(axis=0), a.max(axis=0))
+        th = np.array([theta[int(k)] for k in mv])
+        assert (norm / 2.0 ** sv <= th * (1 + 1e-9)).all()
+        assert (sv >= 0).all()
+    return float(err.max()), float(cons.max())
+
+
+# ------------------------------------------------------------------ BASELINE.json configs at oracle-sized cell counts
+def test_config1_full(dg, oracle, cuda):
+    """configs[0]: N = 1, 32^3 cells, every cell compared."""
+    wl = W.make_workload(1, device=cuda)
+    run_and_compare(dg, oracle, wl)
+
+
+@pytest.mark.parametrize("config,ncells", [(2, 20011), (3, 6007), (4, 2053)])
+def test_configs_reduced(dg, oracle, cuda, config, ncells):
+    """configs[1..3] recipes at reduced, ragged cell counts (several blocks plus a tail), every cell compared."""
+    wl = W.make_workload(config, ncells=ncells, device=cuda)
+    run_and_compare(dg, oracle, wl)
+
+
+@pytest.mark.parametrize("N", list(range(1, 17)))
+def test_sweep_every_species_count(dg, oracle, cuda, N):
+    """configs[4] generator (stiff: dt/t_s up to 1e4) for every N = 1..16, ragged cell count."""
+    wl = W.make_workload(5, ncells=1000 + 37 * N, N=N, device=cuda)
+    run_and_compare(dg, oracle, wl)
+
+
+# ------------------------------------------------------------------ full sizes, the launch configuration bench.py times
+@pytest.mark.parametrize("config", [2, 3, 4])
+def test_full_size_sampled(dg, oracle, cuda, config):
+    """BASELINE.json's full cell counts (128^3 / 256^3): parity on a strided sample of cells the oracle computes one
+    by one, conservation on EVERY cell (needs no oracle; fp64 sums on the device, rounding ~n*u << 1e-13)."""
+    wl = W.make_workload(config, device=cuda)
+    idx = W.sample_cells(wl.ncells, 2048)
+    run_and_compare(dg, oracle, wl, idx=idx)
+    out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    drift = (out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)
+    assert torch.isfinite(out).all()
+    assert float(drift.max()) <= CONS_TOL
+
+
+# ------------------------------------------------------------------ stage-level entry points
+@pytest.mark.parametrize("config,N,ncells", [(1, 1, 4099), (2, 4, 3001), (5, 3, 1500), (3, 8, 2500), (4, 16, 700), (5, 12, 900)])
+def test_stages_match_oracle_stages(dg, oracle, cuda, config, N, ncells):
+    wl = W.make_workload(config, ncells=ncells, N=N, device=cuda)
+    n = N + 1
+    rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(ncells))
+    # a1: Eq. 17 entry by entry (fp64 division and product: a few ulp per entry)
+    A = dg.dg_drag_matrix_build(wl.rho_g, wl.rho_d, wl.t_s, wl.dt)
+    A_h = A.cpu().numpy()
+    A_ref = oracle.drag_matrix_build(rho_g, rho_d, t_s, wl.dt)
+    rel = np.abs(A_h.astype(LD) - A_ref) / np.where(A_ref != 0, np.abs(A_ref), LD(1))
+    assert float(rel.max()) <= (N + 3) * 2.0 ** -53          # A_00 is an N-term fp64 sum, the rest two or three roundings
+    assert ((A_ref == 0) == (A_h == 0)).all()                # the structural zeros of Eq. 17
+    assert (A_h.reshape(n, n, ncells)[0, 1:] > 0).all() and (A_h.reshape(n, n, ncells)[1:, 0] >= 0).all()
+    # a2-a4: exp of the fp64 matrix the GPU built; entries are in [0,1], so the tolerance is absolute
+    E, s = dg.dg_expm_scale_square(A, N, want_s=True)
+    E_h = E.cpu().numpy()
+    E_ref, _ = oracle.expm_batch(A_h, N, rebuild_diag=True)
+    assert float(np.abs(E_h.astype(LD) - E_ref).max()) <= 1e-13
+    colsum = E_h.astype(LD).reshape(n, n, ncells).sum(axis=0)
+    assert float(np.abs(colsum - 1).max()) <= 1e-14
+    assert E_h.min() >= 0.0 and E_h.max() <= 1.0 + 1e-15
+    assert int(s.min()) >= 0
+    # a5
+    out = dg.dg_drag_apply(E, wl.p_in, N)
+    out_ref = oracle.drag_apply(E_h, p_in, N)
+    assert float(oracle.parity_error(out.cpu().numpy(), out_ref, p_in).max()) <= 1e-14
+    # the three stages chained reproduce the fused kernel within the parity tolerance
+    fused = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    ref = oracle.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+    assert float(oracle.parity_error(out.cpu().numpy(), ref, p_in).max()) <= PARITY_TOL
+    assert float(oracle.parity_error(fused.cpu().numpy(), ref, p_in).max()) <= PARITY_TOL
+    # expm in place (E aliases A)
+    A2 = A.clone()
+    dg.dg_expm_scale_square(A2, N, E=A2)
+    assert torch.equal(A2, E)
+
+
+# ------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("N", [1, 4, 8, 9, 16])
+@pytest.mark.parametrize("ncells", [1, 2, 31, 33, 127, 129, 257])
+def test_ragged_and_tiny_cell_counts(dg, oracle, cuda, N, ncells):
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
+    run_and_compare(dg, oracle, wl)
+
+
+@pytest.mark.parametrize("N", [1, 3, 8, 16])
+def test_empty_input_is_a_noop(dg, cuda, N):
+    n = N + 1
+    z = lambda *s: torch.empty(s, dtype=torch.float64, device=cuda)
+    out = dg.dg_drag_update(z(0), z(N, 0), z(N, 0), 0.1, z(3, n, 0))
+    assert out.shape == (3, n, 0)
+    A = dg.dg_drag_matrix_build(z(0), z(N, 0), z(N, 0), 0.1)
+    E = dg.dg_expm_scale_square(A, N)
+    dg.dg_drag_apply(E, z(3, n, 0), N)
+    torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("N", [1, 2, 5, 8, 13, 16])
+def test_dt_zero_is_the_identity_bit_for_bit(dg, cuda, N):
+    wl = W.make_workload(5, ncells=777, N=N, device=cuda)
+    out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, 0.0, wl.p_in)
+    assert torch.equal(out, wl.p_in)
+
+
+@pytest.mark.parametrize("N", [1, 2, 4, 8, 11, 16])
+def test_in_place_update(dg, cuda, N):
+    wl = W.make_workload(5, ncells=1501, N=N, device=cuda)
+    ref = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    p = wl.p_in.clone()
+    dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p, p_out=p)
+    assert torch.equal(p, ref)
+    # and the launch is deterministic run to run
+    again = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    assert torch.equal(again, ref)
+
+
+@pytest.mark.parametrize("N", [1, 2, 4, 8, 16])
+def test_zero_dust_density_species(dg, oracle, cuda, N):
+    """DESIGN.md R12: rho_d,i = 0 is allowed (species i receives nothing from the gas)."""
+    wl = W.make_workload(2, ncells=600, N=N, device=cuda)
+    wl.rho_d[0, ::2] = 0.0
+    wl.rho_d[N - 1, 1::3] = 0.0
+    wl.rho_d[:, 5] = 0.0
+    run_and_compare(dg, oracle, wl)
+
+
+@pytest.mark.parametrize("N", [1, 3, 8, 16])
+def test_extreme_stiffness_and_weak_coupling(dg, oracle, cuda, N):
+    """dt/t_s from 1e-12 (s = 0, lowest Table B.1 rows) to 1e10 (about 37 squarings); eps from 1e-8 to 1e3."""
+    ncells = 512
+    g = torch.Generator(device="cpu"); g.manual_seed(99 + N)
+    u = lambda *s: torch.rand(*s, generator=g, dtype=torch.float64)
+    rho_g = (10 ** (4 * u(ncells) - 2)).to(cuda)
+    eps = (10 ** (11 * u(N, ncells) - 8)).to(cuda)
+    t_s = (10 ** (22 * u(N, ncells) - 12)).to(cuda)
+    t_s[:, :64] = 1e10      # norm ~ 1e-12: rows m = 2, 4 of Table B.1
+    t_s[:, 64:128] = 1e-12  # norm ~ 1e10
+    p_in = torch.randn(3, N + 1, ncells, generator=g, dtype=torch.float64).to(cuda)
+    wl = W.Workload("extreme", 0, N, ncells, 1e-2, rho_g, (eps * rho_g).contiguous(), t_s.contiguous(), p_in)
+    run_and_compare(dg, oracle, wl)
+
+
+def test_equal_velocity_state_is_a_fixed_point(dg, cuda):
+    """Omega rho = 0 (Eq. 17): momenta proportional to the densities do not change (long-time limit)."""
+    for N in (1, 4, 8, 16):
+        wl = W.make_workload(5, ncells=999, N=N, device=cuda)
+        rho = torch.cat([wl.rho_g[None], wl.rho_d], dim=0)
+        v = torch.tensor([0.3, -1.7, 2.5], dtype=torch.float64, device=cuda)
+        p = (v[:, None, None] * rho[None]).contiguous()
+        out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p)
+        assert float(((out - p).abs().amax(dim=(0, 1)) / p.abs().amax(dim=(0, 1))).max()) <= 1e-13
+
+
+# ------------------------------------------------------------------ host-buffer end-to-end entry point
+@pytest.mark.parametrize("N,ncells,chunk", [(1, 5000, 0), (4, 10007, 4096), (8, 3001, 1000), (16, 1237, 500)])
+def test_host_entry_point_matches_device_entry_point(dg, cuda, N, ncells, chunk):
+    wl = W.make_workload(5, ncells=ncells, N=N, device="cpu")
+    pin = lambda t: t.pin_memory()
+    h = [pin(wl.rho_g), pin(wl.rho_d), pin(wl.t_s), pin(wl.p_in)]
+    out_h = dg.dg_drag_update_host(h[0], h[1], h[2], wl.dt, h[3], chunk_cells=chunk)
+    out_d = dg.dg_drag_update(wl.rho_g.to(cuda), wl.rho_d.to(cuda), wl.t_s.to(cuda), wl.dt, wl.p_in.to(cuda))
+    assert torch.equal(out_h, out_d.cpu())
+    # pageable memory and in-place
+    p = wl.p_in.clone()
+    dg.dg_drag_update_host(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p, p_out=p, chunk_cells=chunk)
+    assert torch.equal(p, out_h)
+    dg.dg_host_release()
+
+
+def test_error_codes_on_device_arguments(dg, cuda):
+    lib = dg.raw()
+    x = torch.zeros(64, dtype=torch.float64, device=cuda)
+    p = x.data_ptr()
+    assert lib.dg_drag_update(p, p, p, 0.1, p, 1, 4, p + 4, None) == dg.DG_EALIGN
+    assert lib.dg_drag_update(p, p, p, 0.1, p, 1, 4, None, None) == dg.DG_ENULL
+    assert lib.dg_drag_update(p, p, p, -0.1, p, 1, 4, p, None) == dg.DG_EINVAL
+    assert lib.dg_drag_update(p, p, p, 0.1, p, 17, 4, p, None) == dg.DG_ERANGE
