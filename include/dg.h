@@ -87,6 +87,19 @@ dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const doub
                             const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                             void* stream);
 
+/* Same as dg_drag_update_ex with the thread mapping forced (for measuring the mappings against each other; both
+ * compute the same arithmetic and agree to rounding):
+ *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)
+ *   DG_VARIANT_TPC      thread-per-cell: one thread owns a cell, packed symmetric matrices in registers
+ *   DG_VARIANT_WPC      warp-per-cell: one warp owns a cell, fp64 tensor-core (DMMA) tiles for the squarings
+ * Any other value is DG_EINVAL. */
+#define DG_VARIANT_DEFAULT 0
+#define DG_VARIANT_TPC 1
+#define DG_VARIANT_WPC 2
+dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                                 const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
+                                 int variant, void* stream);
+
 /* ---- the same update on HOST buffers (end-to-end path) -------------------------------------------------------
  * All array arguments are HOST pointers in the layouts above.  The call cuts the cells into chunks of
  * `chunk_cells` (0 = library default), copies each chunk's inputs to a private device staging area, runs the

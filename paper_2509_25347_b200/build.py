@@ -36,6 +36,7 @@ def _units():
     units = [("dg_api.o", "dg_api.cu", []), ("dg_peaks.o", "dg_peaks.cu", []), ("dg_host.o", "dg_host.cu", [])]
     for n in range(1, NMAX + 1):
         units.append((f"dg_kernels_N{n}.o", "dg_kernels.cu", [f"-DDG_N={n}"]))
+        units.append((f"dg_wpc_kernels_N{n}.o", "dg_wpc_kernels.cu", [f"-DDG_N={n}"]))
     return units
 
 

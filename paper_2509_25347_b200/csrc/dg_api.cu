@@ -14,6 +14,18 @@ static const Launchers* const kTable[DG_NMAX + 1] = {
     &launchers_N6,  &launchers_N7,  &launchers_N8,  &launchers_N9,  &launchers_N10, &launchers_N11,
     &launchers_N12, &launchers_N13, &launchers_N14, &launchers_N15, &launchers_N16};
 
+static const WpcLaunchers* const kWpcTable[DG_NMAX + 1] = {
+    nullptr,            &wpc_launchers_N1,  &wpc_launchers_N2,  &wpc_launchers_N3,  &wpc_launchers_N4,
+    &wpc_launchers_N5,  &wpc_launchers_N6,  &wpc_launchers_N7,  &wpc_launchers_N8,  &wpc_launchers_N9,
+    &wpc_launchers_N10, &wpc_launchers_N11, &wpc_launchers_N12, &wpc_launchers_N13, &wpc_launchers_N14,
+    &wpc_launchers_N15, &wpc_launchers_N16};
+
+// The mapping dg_drag_update uses for each N, chosen from measurements on B200: registers hold the
+// packed symmetric matrices of one cell per thread up to N = 12; beyond that the thread-per-cell kernel spills and the
+// warp-per-cell DMMA kernel wins.
+constexpr int kFirstWpcN = 13;
+static inline int default_variant(int N) { return N >= kFirstWpcN ? DG_VARIANT_WPC : DG_VARIANT_TPC; }
+
 static thread_local char g_cuda_err[256] = "";
 
 dg_status cuda_status(cudaError_t e) {
@@ -32,7 +44,10 @@ static dg_status check_common(int N, long long ncells, bool* noop) {
     return DG_OK;
 }
 
-const Launchers* launchers_for(int N) { return (N >= 1 && N <= DG_NMAX) ? kTable[N] : nullptr; }
+cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st) {
+    if (variant == DG_VARIANT_DEFAULT) variant = default_variant(N);
+    return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
+}
 
 }  // namespace dg
 
@@ -74,7 +89,8 @@ dg_status dg_expm_scale_square(const double* A, int N, long long ncells, double*
     DG_CHECK_PTR(E);
     DG_CHECK_OPT_PTR(s_out);
     ExpmArgs a{A, ncells, E, s_out};
-    return cuda_status(kTable[N]->expm(a, static_cast<cudaStream_t>(stream)));
+    cudaStream_t cs = static_cast<cudaStream_t>(stream);
+    return cuda_status(default_variant(N) == DG_VARIANT_WPC ? kWpcTable[N]->expm(a, cs) : kTable[N]->expm(a, cs));
 }
 
 dg_status dg_drag_apply(const double* E, const double* p_in, int N, long long ncells, double* p_out, void* stream) {
@@ -89,13 +105,14 @@ dg_status dg_drag_apply(const double* E, const double* p_in, int N, long long nc
     return cuda_status(kTable[N]->apply(a, static_cast<cudaStream_t>(stream)));
 }
 
-dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const double* t_s, double dt,
-                            const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
-                            void* stream) {
+dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                                 const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
+                                 int variant, void* stream) {
     bool noop;
     dg_status st = check_common(N, ncells, &noop);
     if (st != DG_OK) return st;
     if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
+    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_WPC) return DG_EINVAL;
     if (noop) return DG_OK;
     DG_CHECK_PTR(rho_g);
     DG_CHECK_PTR(rho_d);
@@ -105,7 +122,14 @@ dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const doub
     DG_CHECK_OPT_PTR(s_out);
     DG_CHECK_OPT_PTR(m_out);
     UpdateArgs a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, s_out, m_out};
-    return cuda_status(kTable[N]->update(a, static_cast<cudaStream_t>(stream)));
+    return cuda_status(launch_update(N, variant, a, static_cast<cudaStream_t>(stream)));
+}
+
+dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                            const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
+                            void* stream) {
+    return dg_drag_update_variant(rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, s_out, m_out, DG_VARIANT_DEFAULT,
+                                  stream);
 }
 
 dg_status dg_drag_update(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
@@ -120,7 +144,7 @@ int dg_launches_per_update(int N, long long ncells) {
 
 const char* dg_variant_name(int N) {
     if (N < 1 || N > DG_NMAX) return "";
-    return kTable[N]->variant;
+    return default_variant(N) == DG_VARIANT_WPC ? kWpcTable[N]->variant : kTable[N]->variant;
 }
 
 const char* dg_status_string(dg_status st) {

@@ -14,7 +14,7 @@
 
 namespace dg {
 dg_status cuda_status(cudaError_t e);
-const Launchers* launchers_for(int N);
+cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st);
 
 namespace {
 
@@ -58,7 +58,7 @@ cudaError_t ensure(Ctx& c, size_t bytes) {
     return cudaSuccess;
 }
 
-cudaError_t run(Ctx& c, const Launchers* L, const double* rho_g, const double* rho_d, const double* t_s, double dt,
+cudaError_t run(Ctx& c, const double* rho_g, const double* rho_d, const double* t_s, double dt,
                 const double* p_in, int N, long long ncells, double* p_out, long long chunk) {
     const int n = N + 1;
     const size_t doubles_per_cell = (size_t)(1 + 2 * N + 3 * n + 3 * n);
@@ -79,7 +79,7 @@ cudaError_t run(Ctx& c, const Launchers* L, const double* rho_g, const double* r
         DG_TRY(cudaMemcpy2DAsync(d_t_s, w, t_s + c0, hpitch, w, (size_t)N, cudaMemcpyHostToDevice, s.stream));
         DG_TRY(cudaMemcpy2DAsync(d_p_in, w, p_in + c0, hpitch, w, (size_t)3 * n, cudaMemcpyHostToDevice, s.stream));
         UpdateArgs a{d_rho_g, d_rho_d, d_t_s, dt, d_p_in, cc, d_p_out, nullptr, nullptr};
-        DG_TRY(L->update(a, s.stream));
+        DG_TRY(launch_update(N, DG_VARIANT_DEFAULT, a, s.stream));
         DG_TRY(cudaMemcpy2DAsync(p_out + c0, hpitch, d_p_out, w, w, (size_t)3 * n, cudaMemcpyDeviceToHost, s.stream));
     }
     for (int j = 0; j < kSlots; ++j) DG_TRY(cudaStreamSynchronize(c.slot[j].stream));
@@ -114,7 +114,7 @@ extern "C" dg_status dg_drag_update_host(const double* rho_g, const double* rho_
     }
     long long chunk = chunk_cells > 0 ? chunk_cells : kDefaultChunk;
     if (chunk > ncells) chunk = ncells;
-    e = run(g_ctx[device], launchers_for(N), rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, chunk);
+    e = run(g_ctx[device], rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, chunk);
     if (device != prev) cudaSetDevice(prev);
     return cuda_status(e);
 }

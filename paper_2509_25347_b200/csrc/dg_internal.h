@@ -45,7 +45,16 @@ struct Launchers {
     const char* variant;
 };
 
-#define DG_DECL_LAUNCHERS(NN) extern const Launchers launchers_N##NN;
+// Warp-per-cell DMMA variant (dg_wpc_kernels.cu, one translation unit per N).
+struct WpcLaunchers {
+    cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    cudaError_t (*expm)(const ExpmArgs&, cudaStream_t);
+    const char* variant;
+};
+
+#define DG_DECL_LAUNCHERS(NN)                 \
+    extern const Launchers launchers_N##NN;   \
+    extern const WpcLaunchers wpc_launchers_N##NN;
 DG_DECL_LAUNCHERS(1)
 DG_DECL_LAUNCHERS(2)
 DG_DECL_LAUNCHERS(3)

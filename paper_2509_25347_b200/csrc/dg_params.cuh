@@ -58,4 +58,11 @@ __device__ __forceinline__ void choose_m_s(double norm, float hcost, int& m, int
     s = min(s, kSMax);
 }
 
+// 1/sqrt(eps) and sqrt(eps) with eps clamped away from zero so that rho_d = 0 stays finite (R12).
+__device__ __forceinline__ void sym_weights(double eps, double& w, double& iw) {
+    eps = fmax(eps, 1e-200);
+    iw = rsqrt(eps);
+    w = eps * iw;
+}
+
 }  // namespace dg

@@ -130,11 +130,4 @@ struct Tpc {
     }
 };
 
-// 1/sqrt(eps) and sqrt(eps) with eps clamped away from zero so that rho_d = 0 stays finite (R12).
-__device__ __forceinline__ void sym_weights(double eps, double& w, double& iw) {
-    eps = fmax(eps, 1e-200);
-    iw = rsqrt(eps);
-    w = eps * iw;
-}
-
 }  // namespace dg

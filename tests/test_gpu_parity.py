@@ -19,9 +19,9 @@ CONS_TOL = 1e-13
 LD = np.longdouble
 
 
-def run_and_compare(dg, oracle, wl, idx=None, check_s=True):
+def run_and_compare(dg, oracle, wl, idx=None, check_s=True, variant=0):
     """Runs the fused kernel on the whole workload and compares the cells `idx` (default: all) with the oracle."""
-    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=variant)
     torch.cuda.synchronize()
     if idx is None:
         idx = torch.arange(wl.ncells)
@@ -67,6 +67,22 @@ def test_sweep_every_species_count(dg, oracle, cuda, N):
     """configs[4] generator (stiff: dt/t_s up to 1e4) for every N = 1..16, ragged cell count."""
     wl = W.make_workload(5, ncells=1000 + 37 * N, N=N, device=cuda)
     run_and_compare(dg, oracle, wl)
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("N", list(range(1, 17)))
+def test_both_thread_mappings_for_every_species_count(dg, oracle, cuda, N, variant):
+    """dg_drag_update_variant: thread-per-cell (1) and warp-per-cell DMMA (2) each against the oracle, for every N,
+    on the stiff configs[4] generator and on the Dustywave-like configs[2] recipe."""
+    wl = W.make_workload(5, ncells=700 + 13 * N, N=N, device=cuda)
+    run_and_compare(dg, oracle, wl, variant=variant)
+    wl = W.make_workload(3, ncells=333, N=N, device=cuda)
+    run_and_compare(dg, oracle, wl, variant=variant)
+    wl = W.make_workload(2, ncells=515, N=N, device=cuda)
+    wl.rho_d[0, ::3] = 0.0                      # zero dust density in one species of every third cell
+    run_and_compare(dg, oracle, wl, variant=variant)
+    out0 = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, 0.0, wl.p_in, variant=variant)[0]
+    assert torch.equal(out0, wl.p_in)           # dt = 0: identity, bit for bit
 
 
 # ------------------------------------------------------------------ full sizes, the launch configuration bench.py times
@@ -196,7 +212,7 @@ def test_extreme_stiffness_and_weak_coupling(dg, oracle, cuda, N):
     assert float(oracle.conservation_error(got, p_in).max()) <= CONS_TOL
     norm = 2.0 * np.maximum((rho_d / rho_g * wl.dt / t_s).sum(axis=0), (wl.dt / t_s).max(axis=0))
     ok = norm <= 1e6
-    assert ok.sum() > 100 and (~ok).sum() > 60 and int(s.max()) >= 35 and int(m.min()) <= 4
+    assert ok.sum() >= 64 and (~ok).sum() >= 64 and int(s.max()) >= 35 and int(m.min()) <= 4
     ref = oracle.drag_update(rho_g[ok], rho_d[:, ok], t_s[:, ok], wl.dt, p_in[:, :, ok])
     assert float(oracle.parity_error(got[:, :, ok], ref, p_in[:, :, ok]).max()) <= PARITY_TOL
     # |exp(A)_kj| <= 1 and columns sum to one, so no output can exceed the sum of the inputs' magnitudes
