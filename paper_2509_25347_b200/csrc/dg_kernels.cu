@@ -19,47 +19,104 @@ constexpr int SZ = Core::SZ;
 constexpr int kThreads = 128;
 
 // ---------------------------------------------------------------------------------------------- fused a1..a5
-__global__ void __launch_bounds__(kThreads) k_update(UpdateArgs g) {
-    const long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
-    if (c >= g.ncells) return;
+// Persistent over cells: thread t of the grid walks cells t, t + T, t + 2T, ... (T = threads in the grid), so a warp
+// always owns 32 consecutive cells and every row access is 256 contiguous bytes.  All global reads go through
+// cp.async (LDGSTS) into the thread's own column of a shared-memory staging tile [row][thread]:
+//   * the momenta of the current cell are requested BEFORE the matrix work and read after it,
+//   * the densities / stopping times of the NEXT cell are requested before the matrix work of the current one,
+// so the few resident warps (the matrices occupy up to 255 registers per thread) never wait on HBM latency.
+// A thread only ever reads shared memory that its own cp.async wrote: cp.async.wait_group is the only
+// synchronisation needed, there is no barrier.
+constexpr int kMinBlocks = N <= 2 ? 8 : N <= 4 ? 4 : N <= 7 ? 3 : 2;  // register budget 64 / 128 / 168 / 255 per thread
+constexpr int kRowsIn = 1 + 2 * N;  // rho_g, rho_d[N], t_s[N]
+constexpr int kRowsP = 3 * n;       // p_in[3][n]
+constexpr size_t kSmemBytes = (size_t)(kRowsIn + kRowsP) * kThreads * sizeof(double);
+
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int Pending>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(Pending) : "memory");
+}
+
+__global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
+    extern __shared__ double stage[];
+    double* s_in = stage + threadIdx.x;                      // [kRowsIn][kThreads]
+    double* sp = stage + kRowsIn * kThreads + threadIdx.x;  // [kRowsP][kThreads]
     const long long nc = g.ncells;
+    const long long stride = (long long)gridDim.x * kThreads;
+    long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
 
-    // a1: eps_i (Eq. 14), a_i = dt alpha_i (Eq. 15), symmetrising weights
-    double a[N], w[N], iw[N];
-    {
-        const double irg = 1.0 / __ldg(g.rho_g + c);
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-            a[i] = g.dt / __ldg(g.t_s + i * nc + c);
-            sym_weights(__ldg(g.rho_d + i * nc + c) * irg, w[i], iw[i]);
+    auto request_inputs = [&](long long cc) {
+        if (cc < nc) {
+            cp_async8(s_in, g.rho_g + cc);
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                cp_async8(s_in + (1 + i) * kThreads, g.rho_d + i * nc + cc);
+                cp_async8(s_in + (1 + N + i) * kThreads, g.t_s + i * nc + cc);
+            });
         }
-    }
-    // a2-a4
-    double P[SZ];
-    int m, s;
-    Core::expm(a, w, iw, P, m, s);
-    if (g.s_out) g.s_out[c] = s;
-    if (g.m_out) g.m_out[c] = m;
+        cp_async_commit();
+    };
+    request_inputs(c);
+    while (c < nc) {
+        static_for<0, kRowsP>([&](auto R) {
+            constexpr int r = R;
+            cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
+        });
+        cp_async_commit();
+        cp_async_wait<1>();  // the inputs of cell c have landed (its momenta may still be in flight)
 
-    // a5: p_out = p_in + W P W^-1 p_in, one component at a time
+        // a1: eps_i (Eq. 14), a_i = dt alpha_i (Eq. 15), symmetrising weights
+        double a[N], w[N], iw[N];
+        {
+            const double irg = 1.0 / s_in[0];
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                a[i] = g.dt / s_in[(1 + N + i) * kThreads];
+                sym_weights(s_in[(1 + i) * kThreads] * irg, w[i], iw[i]);
+            });
+        }
+        const long long cn = c + stride;
+        request_inputs(cn);  // always commits a group (an empty one past the end) so the wait counts stay uniform
+
+        // a2-a4
+        double P[SZ];
+        int m, s;
+        Core::expm(a, w, iw, P, m, s);
+        if (g.s_out) g.s_out[c] = s;
+        if (g.m_out) g.m_out[c] = m;
+
+        // a5: p_out = p_in + W P W^-1 p_in, one component at a time
+        cp_async_wait<1>();  // the momenta of cell c have landed (the next cell's inputs may still be in flight)
 #pragma unroll 1
-    for (int comp = 0; comp < 3; ++comp) {
-        const double* pi = g.p_in + (long long)comp * n * nc + c;
-        double* po = g.p_out + (long long)comp * n * nc + c;
-        double p[n], q[n];
-#pragma unroll
-        for (int k = 0; k < n; ++k) {
-            p[k] = __ldg(pi + k * nc);
-            q[k] = (k == 0) ? p[k] : p[k] * iw[k == 0 ? 0 : k - 1];
+        for (int comp = 0; comp < 3; ++comp) {
+            const double* pi = sp + comp * n * kThreads;
+            double* po = g.p_out + (long long)comp * n * nc + c;
+            double p[n], q[n];
+            static_for<0, n>([&](auto K) {
+                constexpr int k = K;
+                p[k] = pi[k * kThreads];
+                if constexpr (k == 0) q[k] = p[k];
+                else q[k] = p[k] * iw[k - 1];
+            });
+            static_for<0, n>([&](auto I) {
+                constexpr int i = I;
+                double y = 0.0;
+                static_for<0, n>([&](auto K) {
+                    constexpr int k = K;
+                    y = fma(P[Core::sx(i, k)], q[k], y);
+                });
+                if constexpr (i == 0) po[0] = p[0] + y;
+                else po[i * nc] = fma(w[i - 1], y, p[i]);
+            });
         }
-#pragma unroll
-        for (int i = 0; i < n; ++i) {
-            double y = 0.0;
-#pragma unroll
-            for (int k = 0; k < n; ++k) y = fma(P[Core::sx(i, k)], q[k], y);
-            po[i * nc] = (i == 0) ? p[i] + y : fma(w[i == 0 ? 0 : i - 1], y, p[i]);
-        }
+        c = cn;
     }
+    cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------------------------------------- staged a1
@@ -102,16 +159,17 @@ __global__ void __launch_bounds__(kThreads) k_expm(ExpmArgs g) {
     Core::expm(a, w, iw, P, m, s);
     if (g.s_out) g.s_out[c] = s;
     double* E = g.E + c;
-#pragma unroll
-    for (int i = 0; i < n; ++i)
-#pragma unroll
-        for (int k = 0; k < n; ++k) {
+    static_for<0, n>([&](auto I) {
+        constexpr int i = I;
+        static_for<0, n>([&](auto K) {
+            constexpr int k = K;
             double v = P[Core::sx(i, k)];
-            if (i > 0) v *= w[i == 0 ? 0 : i - 1];
-            if (k > 0) v *= iw[k == 0 ? 0 : k - 1];
-            if (i == k) v = 1.0 + P[Core::ix(i, i)];
+            if constexpr (i > 0) v *= w[i - 1];
+            if constexpr (k > 0) v *= iw[k - 1];
+            if constexpr (i == k) v = 1.0 + P[Core::ix(i, i)];
             E[(long long)(i * n + k) * nc] = v;
-        }
+        });
+    });
 }
 
 // ---------------------------------------------------------------------------------------------- staged a5
@@ -142,8 +200,26 @@ __global__ void __launch_bounds__(kThreads) k_apply(ApplyArgs g) {
 
 inline unsigned grid_for(long long ncells) { return (unsigned)((ncells + kThreads - 1) / kThreads); }
 
+// Persistent grid: as many blocks as fit on the device at once (or fewer, if there are not enough cells).
 cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    k_update<<<grid_for(a.ncells), kThreads, 0, st>>>(a);
+    static int blocks_per_sm[64] = {0};  // per device; 0 = not yet queried
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (blocks_per_sm[dev] == 0) {
+        e = cudaFuncSetAttribute(k_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        if (e != cudaSuccess) return e;
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update, kThreads, kSmemBytes);
+        if (e != cudaSuccess) return e;
+        blocks_per_sm[dev] = per_sm > 0 ? per_sm : 1;
+    }
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    const long long want = (a.ncells + kThreads - 1) / kThreads;
+    const long long cap = (long long)sms * blocks_per_sm[dev];
+    k_update<<<(unsigned)(want < cap ? want : cap), kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
 }
 cudaError_t launch_build(const BuildArgs& a, cudaStream_t st) {
