@@ -60,18 +60,26 @@ def algorithmic_flops(wl):
     return products * 2.0 * n ** 3 + 6.0 * n * n * wl.ncells, products / wl.ncells
 
 
-def executed_flops(N, s, m):
-    """Flops the thread-per-cell kernel actually issues (FMA = 2), from the per-cell (m, s) it reports: Horner steps in
-    the symmetric packed form, symmetric squarings with the conservation sums, and the apply."""
+def useful_flops(N, s, m):
+    """Flops of the symmetric / sparse formulation of DESIGN.md §3 for the per-cell (m, s) the kernel reports, counted
+    from the recurrences themselves (FMA = 2, add / mul / div / rsqrt = 1) and independent of the thread mapping: no
+    padding, no divergence, no index or data-movement work.  This is the STRICT numerator of the ALU roofline: it can
+    never exceed what the fp64 pipe executed, so the fraction can never exceed 1."""
     n = N + 1
-    tri = n * (n - 1) // 2
-    horner = n * n + (tri + n) * 2 + n          # row 0: n*n FMA; rows >= 1: 2 ops per packed entry; scale
-    square = tri * n + n * n                    # offdiag(X X) upper triangle + conservation sums
-    apply_ = 3 * (n * n + 2 * n)
+    tri = n * (n - 1) // 2                       # strict upper triangle
+    build = (1 + 2 * N) + 3 * N + (3 * N + 2)    # 1/rho_g, dt/t_s, eps; rsqrt, w; norm (N fma + max) and scaling
+    first = 2 * N + 2 + 2 * N                    # al, be, b00 and P = B/m
+    horner = ((2 * N + 1)                        # B_j = B/j
+              + n * (1 + 2 * N)                  # row 0 of B_j P: one mul + N fma per column
+              + (N * (N + 1) // 2) * 3 + N       # rows >= 1, packed: mul + fma per entry, +1 on the diagonal
+              + n)                               # row 0 += B_j
+    conserve = (2 * N + 1) + N * (1 + 2 * (N - 1) + 1)
+    square = n + tri * (1 + 2 * N) + conserve    # 1 + d; offdiag(X X): mul + N fma per entry; diagonal from conservation
+    apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)
     sm = s.double()
     mm = m.double()
-    fma = ((mm - 1).clamp(min=0) * horner + sm * square + apply_ + n * n).sum().item()
-    return 2.0 * fma
+    per_cell = build + first + (mm - 1).clamp(min=0) * horner + tri + conserve + sm * square + apply_
+    return float(per_cell.sum().item())
 
 
 class ClockSampler:
@@ -209,24 +217,46 @@ def measured_peaks_file():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
-def roofline_for(wl, ms_per_launch, alg_flops, peaks, hbm_gbs, hbm_src):
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full summary of this
+    workload (profiles/traffic.csv: workload,kernel,dram_read_bytes,dram_write_bytes,source), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for ln in f:
+            c = ln.strip().split(",")
+            if len(c) >= 4 and c[0] == workload:
+                return float(c[2]) + float(c[3])
+    return None
+
+
+def roofline_for(wl, ms_per_launch, dense_flops, flops, peaks, hbm_gbs, hbm_src):
     """The binding roofline of the fused kernel: whichever of (algorithmic bytes / HBM peak) and (algorithmic flops /
-    fp64 ALU peak) takes longer."""
+    fp64 ALU peak) takes longer.  `flops` is the strict count of useful_flops(); `dense_flops` is SURVEY.md §8(d)'s
+    dense-product figure F (what Alg. 6-7 of the paper would execute), reported beside it as `dense_equivalent`."""
     nbytes = algorithmic_bytes_per_cell(wl.N) * wl.ncells
+    peak = peaks["fp64_nominal_tflops"]
     t_hbm = nbytes / (hbm_gbs * 1e9)
-    t_alu = alg_flops / (peaks["fp64_nominal_tflops"] * 1e12)
+    t_alu = flops / (peak * 1e12)
     sec = ms_per_launch * 1e-3
+    dense = {"achieved": dense_flops / sec / 1e12, "unit": "TFLOP/s", "frac": dense_flops / sec / 1e12 / peak,
+             "note": "SURVEY.md 8(d) F = [min_k(Pi_mk + s_k)] 2n^3 + 6n^2: the flops of the paper's dense Alg. 6-7; "
+                     "the kernels execute fewer (symmetric squarings, sparse Horner), so this can exceed 1"}
+    traffic = ncu_traffic(wl.name)
     if t_alu >= t_hbm:
-        ach = alg_flops / sec / 1e12
-        peak = peaks["fp64_nominal_tflops"]
-        return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+        ach = flops / sec / 1e12
+        return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "traffic": traffic, "algorithmic_bytes": nbytes,
+                "flops": "useful flops of the symmetric/sparse formulation for the per-cell (m, s) (DESIGN.md §6)",
                 "peak_source": "nominal fp64 FMA peak = SMs x 64 lanes x 2 x clocks.max.sm (DESIGN.md §6); "
                                "measured DFMA microbenchmark in peaks.dfma_tflops",
                 "frac_of_measured_dfma": ach / peaks["dfma_tflops"],
-                "hbm_frac": (nbytes / sec / 1e9) / hbm_gbs}
+                "hbm_frac": (nbytes / sec / 1e9) / hbm_gbs, "dense_equivalent": dense}
     ach = nbytes / sec / 1e9
-    return {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs, "traffic": None,
-            "peak_source": hbm_src, "alu_frac": (alg_flops / sec / 1e12) / peaks["fp64_nominal_tflops"]}
+    return {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
+            "traffic": traffic, "algorithmic_bytes": nbytes, "peak_source": hbm_src,
+            "alu_frac": (flops / sec / 1e12) / peak, "dense_equivalent": dense}
 
 
 def cpu_oracle_sample(wl, budget_s=15.0):
@@ -285,24 +315,20 @@ def run_reference(args):
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
-def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, want_exec=True, sampler=None):
+def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
     p_out = torch.empty_like(wl.p_in)
     total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
-    alg_flops, products = algorithmic_flops(wl)
+    dense_flops, products = algorithmic_flops(wl)
+    _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)  # untimed: per-cell (m, s)
+    flops = useful_flops(wl.N, s, m)
     ms_launch = sum(per) / len(per)
-    roof = roofline_for(wl, ms_launch, alg_flops, peaks, hbm_gbs, hbm_src)
+    roof = roofline_for(wl, ms_launch, dense_flops, flops, peaks, hbm_gbs, hbm_src)
     res = {"workload": wl.name, "N": wl.N, "ncells": wl.ncells, "ms_per_step": total_ms / steps,
            "ms_per_launch_min": min(per), "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
-           "algorithmic_flops_per_cell": alg_flops / wl.ncells, "algorithmic_products_per_cell": products,
-           "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N), "roofline": roof,
-           "variant": dg.dg_variant_name(wl.N)}
-    if want_exec:
-        _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
-        ex = executed_flops(wl.N, s, m)
-        res["executed_flops_per_cell"] = ex / wl.ncells
-        res["executed_tflops"] = ex / (ms_launch * 1e-3) / 1e12
-        res["mean_s"] = float(s.double().mean().item()); res["mean_m"] = float(m.double().mean().item())
-        res["max_s"] = int(s.max().item())
+           "useful_flops_per_cell": flops / wl.ncells, "dense_flops_per_cell": dense_flops / wl.ncells,
+           "dense_products_per_cell": products, "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N),
+           "mean_s": float(s.double().mean().item()), "mean_m": float(m.double().mean().item()),
+           "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
     del p_out
     return res, total_ms
 
