@@ -68,11 +68,11 @@ def useful_flops(N, s, m):
     n = N + 1
     tri = n * (n - 1) // 2                       # strict upper triangle
     build = (1 + 2 * N) + 3 * N + (3 * N + 2)    # 1/rho_g, dt/t_s, eps; rsqrt, w; norm (N fma + max) and scaling
-    first = 2 * N + 2 + 2 * N                    # al, be, b00 and P = B/m
-    horner = ((2 * N + 1)                        # B_j = B/j
-              + n * (1 + 2 * N)                  # row 0 of B_j P: one mul + N fma per column
-              + (N * (N + 1) // 2) * 3 + N       # rows >= 1, packed: mul + fma per entry, +1 on the diagonal
-              + n)                               # row 0 += B_j
+    first = 2 * N + 2 + N                        # al, be, b00 and P = B/m (row 0 only)
+    horner = ((2 * N + 1)                        # B_j = B/j: alpha, beta, b00 scaled
+              + (N * (N - 1) // 2) * 3           # dust block off the diagonal, packed: mul + fma per entry
+              + (2 * N - 1)                      # (B_j P)_00: one mul + (N-1) fma
+              + 1 + 3 * N + 2)                   # 1 + P_00; row 0 from column 0 (mul + fma each); P_00
     conserve = (2 * N + 1) + N * (1 + 2 * (N - 1) + 1)
     square = n + tri * (1 + 2 * N) + conserve    # 1 + d; offdiag(X X): mul + N fma per entry; diagonal from conservation
     apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)

@@ -102,7 +102,8 @@ dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const
 
 /* ---- the same update on HOST buffers (end-to-end path) -------------------------------------------------------
  * All array arguments are HOST pointers in the layouts above.  The call cuts the cells into chunks of
- * `chunk_cells` (0 = library default), copies each chunk's inputs to a private device staging area, runs the
+ * `chunk_cells` (0 = library default; rounded up to a multiple of 256 cells so that the result is bit-identical
+ * to one dg_drag_update launch over all cells), copies each chunk's inputs to a private device staging area, runs the
  * fused kernel and copies the result back, overlapping the three on internal streams; it returns after the last
  * copy has completed (it synchronises).  Page-locked host buffers make the copies truly asynchronous; pageable
  * buffers work but serialise.  p_out may alias p_in.  `device` is the CUDA device ordinal (-1 = current). */

@@ -112,7 +112,11 @@ extern "C" dg_status dg_drag_update_host(const double* rho_g, const double* rho_
         e = cudaSetDevice(device);
         if (e != cudaSuccess) return cuda_status(e);
     }
+    // Chunks are whole multiples of 256 cells: the thread-per-cell kernels take one decision (the Taylor degree) per
+    // warp of 32 consecutive cells, so every chunk must start on the same 32-cell boundaries as a single launch over
+    // all cells for the two entry points to agree bit for bit; 256 also keeps every staged row 2 KiB-aligned.
     long long chunk = chunk_cells > 0 ? chunk_cells : kDefaultChunk;
+    chunk = (chunk + 255) & ~255LL;
     if (chunk > ncells) chunk = ncells;
     e = run(g_ctx[device], rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, chunk);
     if (device != prev) cudaSetDevice(prev);

@@ -14,10 +14,6 @@ __constant__ const int c_m[kRows] = {2, 4, 6, 9, 12, 16, 20, 25, 30};
 __constant__ const double c_theta[kRows] = {2.5809568029e-8, 3.3971688399e-4, 9.0656564075e-3,
                                             8.9577602032e-2, 2.9961589138e-1, 7.8028742566e-1,
                                             1.4382525967,    2.4285825244,    3.5396663487};
-// 1/theta_m (rounded; scaling_exponent() re-checks its result against theta_m itself)
-__constant__ const double c_inv_theta[kRows] = {1.0 / 2.5809568029e-8, 1.0 / 3.3971688399e-4, 1.0 / 9.0656564075e-3,
-                                                1.0 / 8.9577602032e-2, 1.0 / 2.9961589138e-1, 1.0 / 7.8028742566e-1,
-                                                1.0 / 1.4382525967,    1.0 / 2.4285825244,    1.0 / 3.5396663487};
 // 1/j for the Horner recurrence P <- (B + B P)/j, j = 1..30 (index 0 unused)
 __constant__ const double c_inv[31] = {
     0.0,        1.0 / 1.0,  1.0 / 2.0,  1.0 / 3.0,  1.0 / 4.0,  1.0 / 5.0,  1.0 / 6.0,  1.0 / 7.0,
@@ -30,32 +26,58 @@ constexpr int kSMax = 1000;  // 2^-s must stay a normal double
 // 2^-s exactly, 0 <= s <= kSMax
 __device__ __forceinline__ double pow2neg(int s) { return __hiloint2double((1023 - s) << 20, 0); }
 
-// Smallest s >= 0 with norm * 2^-s <= theta (reading R6: the ceil form of Eq. B.10), found
-// from the exponent field of norm/theta plus one compare instead of a rounded log2.
-__device__ __forceinline__ int scaling_exponent(double norm, double theta, double inv_theta) {
-    double r = norm * inv_theta;
-    int e = ((__double2hiint(r) >> 20) & 0x7ff) - 1022;  // r = f * 2^e, f in [0.5, 1), for normal r
-    int s = max(e - 1, 0);                                // norm/2^(e-1) = 2 f theta: may still exceed theta
-    if (norm * pow2neg(min(s, kSMax)) > theta) ++s;
-    return s;
+// Smallest s >= 0 with norm * 2^-s <= theta (reading R6: the ceil form of Eq. B.10), exact
+// and in integer arithmetic.  With norm = f 2^e and theta = g 2^t (f, g in [1, 2)) the answer is e - t + (f > g),
+// which is the carry of the bit patterns' difference: ceil((bits(norm) - bits(theta)) / 2^52).  No rounded log2 and
+// no fp64 instruction.  norm >= 0 and finite; subnormal norms give 0.
+__device__ __forceinline__ int scaling_exponent(double norm, double theta) {
+    const long long d = __double_as_longlong(norm) - __double_as_longlong(theta) + 0xFFFFFFFFFFFFFLL;
+    return max((int)(d >> 52), 0);
 }
 
 // Choice of the Table B.1 row: minimise the cost  hcost * m_k + s_k  over the nine rows (B.11, PAPER.md:635-638,
 // with the polynomial priced by this implementation's sparse Horner recurrence, hcost = cost of one Horner step in
 // units of one squaring, instead of Pi_m dense products; reading R8).  Ties go to the lower row.
-// Non-finite norms give s = 0 (the NaN/Inf then propagates through the polynomial into that cell's output only).
-__device__ __forceinline__ void choose_m_s(double norm, float hcost, int& m, int& s) {
-    m = c_m[kRows - 1];
-    s = 0;
-    if (!(norm <= 1.7e308)) return;
+// Non-finite norms give row 8 (m = 30).
+__device__ __forceinline__ int choose_row(double norm, float hcost) {
+    int row = kRows - 1;
+    if (!(norm <= 1.7e308)) return row;
     float best = 3.0e38f;
 #pragma unroll
     for (int k = 0; k < kRows; ++k) {
-        int sk = scaling_exponent(norm, c_theta[k], c_inv_theta[k]);
+        int sk = scaling_exponent(norm, c_theta[k]);
         float cost = hcost * (float)c_m[k] + (float)sk;
-        if (cost < best) { best = cost; m = c_m[k]; s = sk; }
+        if (cost < best) { best = cost; row = k; }
     }
-    s = min(s, kSMax);
+    return row;
+}
+
+// s for a given row; a non-finite norm gives s = 0 (the NaN/Inf then propagates through the polynomial into that
+// cell's output only).
+__device__ __forceinline__ int s_for_row(double norm, int row) {
+    if (!(norm <= 1.7e308)) return 0;
+    return min(scaling_exponent(norm, c_theta[row]), kSMax);
+}
+
+// One cell decides alone (warp-per-cell mapping, where the whole warp holds the same norm).
+__device__ __forceinline__ void choose_m_s(double norm, float hcost, int& m, int& s) {
+    const int row = choose_row(norm, hcost);
+    m = c_m[row];
+    s = s_for_row(norm, row);
+}
+
+// Thread-per-cell mapping: the lanes of a warp run the Horner loop in lock step, so a per-lane degree would cost
+// max(m) steps anyway.  The row is therefore chosen ONCE per warp, for the largest norm among the active lanes (the
+// paper rewrites Alg. 1 as the branch-reduced Alg. 2 for the same reason), and every lane then takes
+// the smallest s that satisfies Theorem 1's premise for ITS OWN norm with that row.  Any row is admissible for any
+// cell, so correctness never depends on which lanes took part.  The warp maximum is taken on the high word of the
+// double (one REDUX instruction) and rounded up: an upper bound within 2^-20, which can only cost, never break.
+__device__ __forceinline__ void choose_m_s_warp(double norm, float hcost, int& m, int& s) {
+    const unsigned hi = __reduce_max_sync(__activemask(), (unsigned)__double2hiint(norm));  // NaN / Inf / negative win
+    const double nmax = (hi >= 0x7ff00000u) ? __longlong_as_double(0x7ff0000000000000LL) : __hiloint2double((int)hi + 1, 0);
+    const int row = choose_row(nmax, hcost);
+    m = c_m[row];
+    s = s_for_row(norm, row);
 }
 
 // 1/sqrt(eps) and sqrt(eps) with eps clamped away from zero so that rho_d = 0 stays finite (R12).

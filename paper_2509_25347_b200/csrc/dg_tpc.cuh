@@ -10,7 +10,9 @@
 //     never computed by the recurrences but re-derived from conservation of total momentum (columns of Eq. 17 sum
 //     to zero):   d_j = -(sum_{i != j} w_i O_ij) / w_j.
 //     - Taylor polynomial (Eq. 19) without ever adding I:   P <- B_j + B_j P,  B_j = B / j,  j = m .. 1,
-//       B = S / 2^s, exploiting that B has 3N+1 non-zeros (one Horner step is O(n^2)).
+//       B = S / 2^s.  B has 3N+1 non-zeros, and P is a polynomial in B, so B P = P B is symmetric: row 0 of B P is
+//       its column 0, (B P)_0k = (B P)_k0 = beta_k P_00 - alpha_k P_0k, and only (B P)_00 needs a dot product.  One
+//       Horner step is N^2 + 4N + 3 fp64-pipe instructions.
 //     - Squaring (Eq. 23-24):  O <- offdiag((O + diag(1+d))^2), a sum of non-negative products,
 //       so the s squarings amplify no cancellation error and total momentum is conserved to rounding at every step.
 //   * Apply (Eq. 18):  p_out = p_in + W P W^-1 p_in.
@@ -46,7 +48,7 @@ struct Tpc {
 
     // fp64-pipe instructions of one Horner step and of one squaring (with its conservation sums) as coded below;
     // their ratio prices the polynomial in choose_m_s (R8).
-    static constexpr int kHornerOps = 2 * n * n + 2 * n;
+    static constexpr int kHornerOps = N * N + 4 * N + 3;
     static constexpr int kSquareOps = n * n * (n - 1) / 2 + n * n + n;
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
@@ -71,15 +73,19 @@ struct Tpc {
     // slots = d) and m, s are the chosen Taylor degree and scaling exponent.
     __device__ __forceinline__ static void expm(const double (&a)[N], const double (&w)[N], const double (&iw)[N],
                                                 double (&P)[SZ], int& m, int& s) {
-        // ||A||_1 of Eq. 17 in closed form: column 0 sums to 2 sum_i eps_i a_i, column i to 2 a_i (R5)
+        // The scaling exponent is chosen on ||S||_2 (Theorem 1, holds in any consistent norm; S is
+        // symmetric and the whole iteration runs in S's basis).  S is negative semi-definite and its eigenvalues
+        // -mu solve the secular equation 1 = sum_i eps_i a_i / (mu - a_i) (Eq. 29's lambda), whose
+        // largest root obeys  mu <= max_i a_i + sum_i eps_i a_i  =: norm  (<= ||A||_1 = 2 max(sum eps a, max a);
+        // DESIGN.md R5).
         double sb = 0.0, amax = 0.0;
         static_for<0, N>([&](auto I) {
             constexpr int i = I;
             sb = fma(a[i] * w[i], w[i], sb);
             amax = fmax(amax, a[i]);
         });
-        const double norm = 2.0 * fmax(sb, amax);
-        choose_m_s(norm, hcost(), m, s);
+        const double norm = sb + amax;
+        choose_m_s_warp(norm, hcost(), m, s);  // m is warp-uniform, s is this cell's own
         const double sc = pow2neg(s);
 
         double al[N], be[N];
@@ -100,10 +106,9 @@ struct Tpc {
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
                 P[ix(0, i)] = be[i - 1] * r;
-                P[ix(i, i)] = -al[i - 1] * r;
             });
         }
-        // P <- B_j + B_j P,  B_j = B / j
+        // P <- B_j + B_j P,  B_j = B / j.  Every right-hand side below uses the OLD row 0 of P.
         for (int j = m - 1; j >= 1; --j) {
             const double r = c_inv[j];
             double alj[N], bej[N];
@@ -112,32 +117,29 @@ struct Tpc {
                 alj[i] = al[i] * r;
                 bej[i] = be[i] * r;
             });
-            const double b00j = b00 * r;
-            double t[n];  // row 0 of B_j P, from the old P
-            static_for<0, n>([&](auto K) {
-                constexpr int k = K;
-                double acc = b00j * P[ix(0, k)];
-                static_for<1, n>([&](auto L) {
-                    constexpr int l = L;
-                    acc = fma(bej[l - 1], P[sx(l, k)], acc);
-                });
-                t[k] = acc;
-            });
-            static_for<1, n>([&](auto I) {  // rows i >= 1: (B_j P)_ik = beta_i P_0k - alpha_i P_ik, plus B_j itself
+            // dust block, i >= 1, off the diagonal: (B_j P)_ik = beta_i P_0k - alpha_i P_ik.  The dust DIAGONAL is not
+            // carried through the polynomial at all: a Horner step feeds P_ii only back into P_ii, and the final
+            // diagonal is re-derived from conservation below.
+            static_for<1, n>([&](auto I) {
                 constexpr int i = I;
-                static_for<i, n>([&](auto K) {
+                static_for<i + 1, n>([&](auto K) {
                     constexpr int k = K;
-                    if constexpr (k == i)
-                        P[ix(i, i)] = fma(bej[i - 1], P[ix(0, i)], -alj[i - 1] * (P[ix(i, i)] + 1.0));
-                    else
-                        P[ix(i, k)] = fma(bej[i - 1], P[ix(0, k)], -alj[i - 1] * P[ix(i, k)]);
+                    P[ix(i, k)] = fma(bej[i - 1], P[ix(0, k)], -alj[i - 1] * P[ix(i, k)]);
                 });
             });
-            P[ix(0, 0)] = b00j + t[0];
+            // (B_j P)_00 = b00_j P_00 + sum_l beta_l P_l0
+            double t00 = bej[0] * P[ix(0, 1)];
+            static_for<2, n>([&](auto L) {
+                constexpr int l = L;
+                t00 = fma(bej[l - 1], P[ix(0, l)], t00);
+            });
+            // row 0, k >= 1, from column 0 of the symmetric product: beta_k P_00 - alpha_k P_0k, plus B_j's beta_k
+            const double x00 = 1.0 + P[ix(0, 0)];
             static_for<1, n>([&](auto K) {
                 constexpr int k = K;
-                P[ix(0, k)] = bej[k - 1] + t[k];
+                P[ix(0, k)] = fma(bej[k - 1], x00, -alj[k - 1] * P[ix(0, k)]);
             });
+            P[ix(0, 0)] = fma(b00 * r, x00, t00);
         }
         // off-diagonals are non-negative in exact arithmetic; clamp the rounding noise, then re-derive the diagonal
         static_for<0, n>([&](auto I) {

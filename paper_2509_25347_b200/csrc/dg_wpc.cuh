@@ -2,9 +2,9 @@
 // warp's registers in the fp64 tensor-core accumulator layout and is squared with DMMA (mma.sync m8n8k4 f64).
 //
 // Same arithmetic as dg_tpc.cuh (symmetrised arrowhead S = W^-1 (dt Omega) W, P = exp(S) - I = O + diag(d), Taylor
-// recurrence P <- (B + B P)/j, cancellation-free squarings with the diagonal re-derived from conservation of total
-// momentum); only the mapping differs.  This is the "hierarchical" kernel the paper suggests but does not build
-// (PAPER.md:329, 343).
+// recurrence P <- (B + B P)/j with B P = P B, cancellation-free squarings with the diagonal re-derived from
+// conservation of total momentum); only the mapping differs.  This is the "hierarchical" kernel the paper suggests
+// but does not build.
 //
 // Layout.  The symmetric matrix X = [[x00, r^T], [r, D]] is split into the gas entry x00, the gas-dust vector r and
 // the ND x ND dust block D (ND = 8 or 16, species beyond N are zero padding that stays decoupled).  With lane
@@ -13,9 +13,13 @@
 // Because D is symmetric, T[I][K][e] is at the same time the A fragment (rows 8I.., k-set {8K + 2t + e}) and T[J][K][e]
 // the B fragment (k-set {8K + 2t + e}, columns 8J..) of mma.m8n8k4 — the k index may be permuted freely as long as A
 // and B agree — so    (D D)[tile I, J] = sum_{K, e} mma(T[I][K][e], T[J][K][e])    lands directly in the layout the
-// next squaring consumes: no fragment re-layout between squarings.  The rank-one border r r^T is one more mma whose
-// k = 0 slot carries r.  Tile (1,0) is the transpose of tile (0,1), fetched with shuffles instead of five more DMMAs.
+// next squaring consumes: no fragment re-layout between squarings.  The rank-one border r r^T initialises the
+// accumulators (two DMUL per tile: cheaper than a DMMA whose k-slots would be three-quarters empty).  Tile (1,0) is the
+// transpose of tile (0,1), fetched with shuffles instead of four more DMMAs.
 // Vectors come in two replicated forms: row-indexed vR[I] = v[8 I + g] and column-indexed vC[J][e] = v[8 J + 2 t + e].
+//
+// Measured on B200: DMMA.8x8x4 issues every 16 cycles per SM sub-partition (the same 64 FMA/clk/SM as
+// DFMA) with a dependent-accumulator latency of 26 cycles; m16n8k{4,8,16} compile to sequences of DMMA.8x8x4.
 #pragma once
 #include "dg_params.cuh"
 
@@ -34,23 +38,30 @@ __device__ __forceinline__ double quad_sum(double x) {  // over t (lanes 4g .. 4
     x += __shfl_xor_sync(kFull, x, 2);
     return x;
 }
-__device__ __forceinline__ double oct_sum(double x) {  // over g (lanes with equal t)
-    x += __shfl_xor_sync(kFull, x, 4);
-    x += __shfl_xor_sync(kFull, x, 8);
-    x += __shfl_xor_sync(kFull, x, 16);
-    return x;
-}
+
+// Per-cell quantities the canonical lanes prepare in shared memory (species j < N; padding: a = be = 0, w = iw = 1).
+template <int ND>
+struct CellVecs {
+    double a[ND];   // dt / t_s,j                       (Eq. 15)
+    double be[ND];  // a_j sqrt(eps_j)
+    double w[ND];   // sqrt(eps_j)                      (Eq. 14)
+    double iw[ND];  // 1 / sqrt(eps_j)
+    double sb;      // sum_j eps_j a_j
+    double amax;    // max_j a_j
+};
 
 template <int N>
 struct Wpc {
     static constexpr int n = N + 1;
     static constexpr int TL = (N <= 8) ? 1 : 2;
     static constexpr int ND = 8 * TL;
-    // one Horner step costs about a third of a squaring in this mapping (measured)
-    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.6f : 0.33f; }
+    // fp64-pipe cycles of one Horner step over those of one squaring, as coded below (a DMMA holds the pipe for 16
+    // cycles, every other fp64 instruction for 2): prices the polynomial in choose_m_s (R8)
+    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.45f : 0.25f; }
 
     struct VecR { double v[TL]; };
     struct VecC { double v[TL][2]; };
+    using Cell = CellVecs<ND>;
 
     struct Lane {
         int g, t;
@@ -59,8 +70,8 @@ struct Wpc {
             const int lane = threadIdx.x & 31;
             g = lane >> 2;
             t = lane & 3;
-            dg[0] = (t == (g >> 1)) && ((g & 1) == 0);
-            dg[1] = (t == (g >> 1)) && ((g & 1) == 1);
+            dg[0] = (g == 2 * t);
+            dg[1] = (g == 2 * t + 1);
         }
     };
 
@@ -76,36 +87,45 @@ struct Wpc {
     __device__ __forceinline__ static void matvec(const double (&T)[TL][TL][2], const VecC& x, VecR& y) {
 #pragma unroll
         for (int I = 0; I < TL; ++I) {
-            double acc = 0.0;
+            double acc = T[I][0][0] * x.v[0][0];
+            acc = fma(T[I][0][1], x.v[0][1], acc);
 #pragma unroll
-            for (int J = 0; J < TL; ++J)
+            for (int J = 1; J < TL; ++J)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) acc = fma(T[I][J][e], x.v[J][e], acc);
             y.v[I] = quad_sum(acc);
         }
     }
+    // sum_col x[col] y[col] for column-indexed vectors (every lane receives the full sum)
+    __device__ __forceinline__ static double dotC(const VecC& x, const VecC& y) {
+        double acc = x.v[0][0] * y.v[0][0];
+        acc = fma(x.v[0][1], y.v[0][1], acc);
+#pragma unroll
+        for (int J = 1; J < TL; ++J)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) acc = fma(x.v[J][e], y.v[J][e], acc);
+        return quad_sum(acc);
+    }
 
     // Conservation of total momentum: with O the off-diagonal part (T with zeroed diagonal, r) returns
     //   dR[I] = -(r[row] + sum_col O[row][col] w[col]) / w[row]   and   d0 = -sum_j w_j r_j.
-    __device__ __forceinline__ static void conserve(const double (&T)[TL][TL][2], const VecR& rR, const VecR& wR,
+    __device__ __forceinline__ static void conserve(const double (&T)[TL][TL][2], const VecR& rR, const VecC& rC,
                                                     const VecC& wC, const VecR& iwR, VecR& dR, double& d0) {
         VecR s;
         matvec(T, wC, s);
-        double acc = 0.0;
 #pragma unroll
-        for (int I = 0; I < TL; ++I) {
-            dR.v[I] = -(rR.v[I] + s.v[I]) * iwR.v[I];
-            acc = fma(wR.v[I], rR.v[I], acc);
-        }
-        d0 = -oct_sum(acc);
+        for (int I = 0; I < TL; ++I) dR.v[I] = -(rR.v[I] + s.v[I]) * iwR.v[I];
+        d0 = -dotC(wC, rC);
     }
 
     __device__ __forceinline__ static void set_diag(const Lane& L, double (&T)[TL][TL][2], const VecR& d, double add) {
 #pragma unroll
-        for (int I = 0; I < TL; ++I)
+        for (int I = 0; I < TL; ++I) {
+            const double v = add + d.v[I];
 #pragma unroll
             for (int e = 0; e < 2; ++e)
-                if (L.dg[e]) T[I][I][e] = add + d.v[I];
+                if (L.dg[e]) T[I][I][e] = v;
+        }
     }
     __device__ __forceinline__ static void zero_diag(const Lane& L, double (&T)[TL][TL][2]) {
 #pragma unroll
@@ -115,13 +135,47 @@ struct Wpc {
                 if (L.dg[e]) T[I][I][e] = 0.0;
     }
 
-    // On entry: alR/beR/beC = a_j 2^-s, beta_j = a_j w_j 2^-s (row / column indexed), b00 = -sum_j beta_j w_j,
-    // wR/wC/iwR the symmetrising weights.  On return T (diagonal slots = d), rR, rC, d0 hold P = exp(S) - I.
-    __device__ __forceinline__ static void expm(const Lane& L, int m, int s, const VecR& alR, const VecR& beR,
-                                                const VecC& beC, double b00, const VecR& wR, const VecC& wC,
-                                                const VecR& iwR, double (&T)[TL][TL][2], VecR& rR, VecC& rC,
-                                                double& d0) {
-        // P = B / m
+    // What the apply step needs once P = exp(S) - I is known: the dust block T (diagonal slots = d), the gas-dust
+    // vector r in both forms, the gas entry d0.
+    struct Result {
+        double T[TL][TL][2];
+        VecR rR;
+        VecC rC;
+        double d0;
+        int m, s;
+    };
+
+    // cv: this cell's vectors in shared memory (read-only here).  All 32 lanes call it together.
+    __device__ __forceinline__ static void expm(const Lane& L, const Cell& cv, Result& R) {
+        // ||S||_2 <= max_j a_j + sum_j eps_j a_j (dg_tpc.cuh gives the argument; R5)
+        const double norm = cv.sb + cv.amax;
+        choose_m_s(norm, hcost(), R.m, R.s);
+        const int m = R.m, s = R.s;
+        const double sc = pow2neg(s);
+
+        VecR alR, beR, iwR;
+        VecC beC, wC;
+#pragma unroll
+        for (int I = 0; I < TL; ++I) {
+            const int row = 8 * I + L.g;
+            alR.v[I] = cv.a[row] * sc;
+            beR.v[I] = cv.be[row] * sc;
+            iwR.v[I] = cv.iw[row];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int col = 8 * I + 2 * L.t + e;
+                beC.v[I][e] = cv.be[col] * sc;
+                wC.v[I][e] = cv.w[col];
+            }
+        }
+        const double b00 = -cv.sb * sc;
+        double (&T)[TL][TL][2] = R.T;
+        VecR& rR = R.rR;
+        VecC& rC = R.rC;
+
+        // P = B / m.  The dust diagonal of P is never carried through the polynomial: a Horner step feeds P_ii only
+        // back into P_ii, and the final diagonal is re-derived from conservation anyway; the diagonal slots of T hold
+        // bounded don't-care values until zero_diag() below.
         double p00;
         {
             const double r = c_inv[m];
@@ -131,40 +185,35 @@ struct Wpc {
                 for (int J = 0; J < TL; ++J) T[I][J][0] = T[I][J][1] = 0.0;
                 rR.v[I] = beR.v[I] * r;
             }
-            VecR dinit;
-#pragma unroll
-            for (int I = 0; I < TL; ++I) dinit.v[I] = -alR.v[I] * r;
-            set_diag(L, T, dinit, 0.0);
 #pragma unroll
             for (int J = 0; J < TL; ++J)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) rC.v[J][e] = beC.v[J][e] * r;
             p00 = b00 * r;
         }
-        // P <- (B + B P) / j
+        // P <- (B + B P) / j, with (B P)_0k taken from column 0 of the symmetric product (dg_tpc.cuh)
         for (int j = m - 1; j >= 1; --j) {
             const double r = c_inv[j];
-            VecR t0;  // row 0 of B P (dust part): b00 r_k + sum_l beta_l P_lk
-            matvec(T, beC, t0);
-            double acc = 0.0;
+            VecR aj, bj;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) acc = fma(beR.v[I], rR.v[I], acc);
-            const double t00 = fma(b00, p00, oct_sum(acc));
+            for (int I = 0; I < TL; ++I) {
+                aj.v[I] = alR.v[I] * r;
+                bj.v[I] = beR.v[I] * r;
+            }
+            // dust block: (B_j P)_ik = beta_i P_0k - alpha_i P_ik
 #pragma unroll
-            for (int I = 0; I < TL; ++I) {  // rows >= 1: (B P)_ik = beta_i P_0k - alpha_i P_ik (+ B_ii on the diagonal)
+            for (int I = 0; I < TL; ++I)
 #pragma unroll
                 for (int J = 0; J < TL; ++J)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        double v = fma(beR.v[I], rC.v[J][e], -alR.v[I] * T[I][J][e]);
-                        if (I == J && L.dg[e]) v -= alR.v[I];
-                        T[I][J][e] = v * r;
-                    }
-            }
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = fma(bj.v[I], rC.v[J][e], -aj.v[I] * T[I][J][e]);
+            // (B_j P)_00 = b00_j P_00 + sum_l beta_l P_l0 ;  row 0: beta_k (1 + P_00) - alpha_k P_0k  (old values)
+            const double t00 = dotC(beC, rC) * r;
+            const double x00 = 1.0 + p00;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) rR.v[I] = (beR.v[I] + fma(b00, rR.v[I], t0.v[I])) * r;
+            for (int I = 0; I < TL; ++I) rR.v[I] = fma(bj.v[I], x00, -aj.v[I] * rR.v[I]);
             row_to_col(L, rR, rC);
-            p00 = (b00 + t00) * r;
+            p00 = fma(b00 * r, x00, t00);
         }
         // clamp the off-diagonals (non-negative in exact arithmetic), re-derive the diagonal from conservation
         zero_diag(L, T);
@@ -178,7 +227,8 @@ struct Wpc {
         }
         row_to_col(L, rR, rC);
         VecR dR;
-        conserve(T, rR, wR, wC, iwR, dR, d0);
+        double d0;
+        conserve(T, rR, rC, wC, iwR, dR, d0);
 
         // s squarings of X = O + diag(1 + d)
         for (int it = 0; it < s; ++it) {
@@ -187,22 +237,23 @@ struct Wpc {
             // gas row of X X: x00 r + D r
             VecR rn;
             matvec(T, rC, rn);
-            // dust block of X X: r r^T + D D, upper tiles by DMMA
+            // dust block of X X: r r^T + D D, upper tiles by DMMA on top of the rank-one border
             double C[TL][TL][2];
-            VecR rb;
-#pragma unroll
-            for (int I = 0; I < TL; ++I) rb.v[I] = (L.t == 0) ? rR.v[I] : 0.0;
 #pragma unroll
             for (int I = 0; I < TL; ++I)
 #pragma unroll
                 for (int J = I; J < TL; ++J) {
-                    C[I][J][0] = C[I][J][1] = 0.0;
-#pragma unroll
-                    for (int K = 0; K < TL; ++K)
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) dmma884(C[I][J][0], C[I][J][1], T[I][K][e], T[J][K][e]);
-                    dmma884(C[I][J][0], C[I][J][1], rb.v[I], rb.v[J]);
+                    C[I][J][0] = rR.v[I] * rC.v[J][0];
+                    C[I][J][1] = rR.v[I] * rC.v[J][1];
                 }
+#pragma unroll
+            for (int K = 0; K < TL; ++K)
+#pragma unroll
+                for (int e = 0; e < 2; ++e)
+#pragma unroll
+                    for (int I = 0; I < TL; ++I)
+#pragma unroll
+                        for (int J = I; J < TL; ++J) dmma884(C[I][J][0], C[I][J][1], T[I][K][e], T[J][K][e]);
             if (TL == 2) {  // tile (1,0)[g][2t+e] = tile (0,1)[2t+e][g], held by lane 4 (2t+e) + g/2 in slot g & 1
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
@@ -220,9 +271,10 @@ struct Wpc {
             }
             zero_diag(L, T);
             row_to_col(L, rR, rC);
-            conserve(T, rR, wR, wC, iwR, dR, d0);
+            conserve(T, rR, rC, wC, iwR, dR, d0);
         }
         set_diag(L, T, dR, 0.0);
+        R.d0 = d0;
     }
 };
 

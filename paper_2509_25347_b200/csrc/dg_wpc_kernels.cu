@@ -1,9 +1,11 @@
 // dg_wpc_kernels.cu — warp-per-cell DMMA kernels for ONE species count N = DG_N (compiled once per N).
 //
-// Each warp walks the cells assigned to it (consecutive cells go to the warps of one block, so the 32-byte sectors a
-// warp touches are shared through L1/L2 with its neighbours).  Lane j < N is the "canonical" lane of dust species j:
-// it loads that species' fields, does the divisions / rsqrt once, and stores that species' results; a per-warp
-// shared-memory table hands the values to the lanes that need them in the tensor-core fragment layout.
+// A warp walks GROUPS of kGroup = 4 consecutive cells: one field row of a group is 32 contiguous bytes — exactly one
+// DRAM sector when the row is 32-byte aligned — so every byte the kernel moves is a byte the method needs (a warp
+// that loaded its single cell's fields lane by lane fetched 4-5x the algorithmic bytes, ncu round 1).  All rows of
+// the NEXT group are requested with cp.async into the warp's private double-buffered staging tile before the
+// matrix work of the current group starts; results are staged in shared memory and written back as whole sectors.
+// There is no block-level synchronisation: warps are independent, __syncwarp is the only barrier.
 #include "dg_internal.h"
 #include "dg_wpc.cuh"
 
@@ -21,202 +23,289 @@ constexpr int TL = Core::TL;
 constexpr int ND = Core::ND;
 constexpr int kWarps = 8;
 constexpr int kThreads = 32 * kWarps;
+constexpr int kGroup = 4;             // cells per staged group
+constexpr int kRowsIn = 1 + 2 * N;    // rho_g, rho_d[N], t_s[N]
+constexpr int kRowsP = 3 * n;         // p[3][n]
+constexpr int kRows = kRowsIn + kRowsP;
+constexpr int kPerPass = 32 / ND;     // cells whose species fit the 32 lanes of one prologue pass
 
-struct WarpSmem {
-    double al[ND], be[ND], w[ND], iw[ND];  // per dust species: a 2^-s, beta, sqrt(eps), 1/sqrt(eps)
-    double q[3][ND], q0[3];                // W^-1 p_in per component
-    double y[3][ND], y0[3];                // P W^-1 p_in per component
+struct alignas(16) WarpSmem {
+    double in[2][kRows][kGroup];   // staged inputs, double buffered: [stage][row][cell of the group]
+    double out[kRowsP][kGroup];    // staged results
+    Core::Cell cell[kGroup];       // per-cell vectors prepared by the prologue
+    double q[3][ND], q0[4];        // W^-1 p_in of the current cell, per component (q0[3] pads to 16 bytes)
 };
+static_assert(sizeof(WarpSmem) % 16 == 0, "cp.async 16-byte destinations need 16-byte aligned per-warp tiles");
+constexpr size_t kSmemBytes = sizeof(WarpSmem) * kWarps;
 
-__device__ __forceinline__ double warp_sum(double x) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(kFull, x, o);
-    return x;
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(src_gmem) : "memory");
 }
-__device__ __forceinline__ double warp_max(double x) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(kFull, x, o));
-    return x;
+__device__ __forceinline__ void cp_async8(void* dst_smem, const void* src_gmem) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int Pending>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(Pending) : "memory");
 }
 
-// Everything between "the a_j, eps_j of this cell are known in the canonical lanes" and "P = exp(S) - I is in the
-// fragment registers".  a, eps: this lane's species (lanes >= N: a = 0, eps = 1).
-struct CellState {
-    double T[TL][TL][2];
-    Core::VecR rR, wR, iwR;
-    Core::VecC rC, iwC;
-    double d0;
-    double w, iw;  // canonical lane's own weights
-    int m, s;
-};
+__device__ __forceinline__ const double* row_ptr(const UpdateArgs& g, int r) {
+    const long long nc = g.ncells;
+    if (r == 0) return g.rho_g;
+    if (r < 1 + N) return g.rho_d + (long long)(r - 1) * nc;
+    if (r < kRowsIn) return g.t_s + (long long)(r - 1 - N) * nc;
+    return g.p_in + (long long)(r - kRowsIn) * nc;
+}
 
-__device__ __forceinline__ void cell_expm(const Core::Lane& L, WarpSmem& sm, int lane, double a, double eps,
-                                          CellState& st) {
-    double w = 1.0, iw = 1.0;
-    if (lane < N) sym_weights(eps, w, iw);
-    const double aw = a * w;
-    const double sb = warp_sum(aw * w);
-    const double amax = warp_max(a);
-    choose_m_s(2.0 * fmax(sb, amax), Core::hcost(), st.m, st.s);
-    const double sc = pow2neg(st.s);
-    __syncwarp();
-    if (lane < ND) {
-        sm.al[lane] = a * sc;
-        sm.be[lane] = aw * sc;
-        sm.w[lane] = w;
-        sm.iw[lane] = iw;
-    }
-    __syncwarp();
-    Core::VecR alR, beR;
-    Core::VecC beC, wC;
-#pragma unroll
-    for (int I = 0; I < TL; ++I) {
-        const int row = 8 * I + L.g;
-        alR.v[I] = sm.al[row];
-        beR.v[I] = sm.be[row];
-        st.wR.v[I] = sm.w[row];
-        st.iwR.v[I] = sm.iw[row];
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const int col = 8 * I + 2 * L.t + e;
-            beC.v[I][e] = sm.be[col];
-            wC.v[I][e] = sm.w[col];
-            st.iwC.v[I][e] = sm.iw[col];
+// Requests all rows of the group starting at cell c0 into `dst`.  vec16: every row start is 16-byte aligned
+// (ncells even) and the group is complete, so a row is two 16-byte copies; otherwise element by element.
+__device__ __forceinline__ void request_group(const UpdateArgs& g, double (*dst)[kGroup], long long c0, int lane,
+                                              bool vec16) {
+    const long long nc = g.ncells;
+    if (c0 < nc) {
+        if (vec16 && c0 + kGroup <= nc) {
+            for (int it = lane; it < 2 * kRows; it += 32) {
+                const int r = it >> 1, h = it & 1;
+                cp_async16(&dst[r][2 * h], row_ptr(g, r) + c0 + 2 * h);
+            }
+        } else {
+            for (int it = lane; it < kGroup * kRows; it += 32) {
+                const int r = it >> 2, k = it & 3;
+                if (c0 + k < nc) cp_async8(&dst[r][k], row_ptr(g, r) + c0 + k);
+            }
         }
     }
-    st.w = w;
-    st.iw = iw;
-    Core::expm(L, st.m, st.s, alR, beR, beC, -sb * sc, st.wR, wC, st.iwR, st.T, st.rR, st.rC, st.d0);
+    cp_async_commit();
+}
+
+// Segmented (ND lanes) sum and max.
+__device__ __forceinline__ double seg_sum(double x) {
+#pragma unroll
+    for (int o = 1; o < ND; o <<= 1) x += __shfl_xor_sync(kFull, x, o);
+    return x;
+}
+__device__ __forceinline__ double seg_max(double x) {
+#pragma unroll
+    for (int o = 1; o < ND; o <<= 1) x = fmax(x, __shfl_xor_sync(kFull, x, o));
+    return x;
+}
+
+// a1 for one lane's (cell, species): eps (Eq. 14), a = dt alpha (Eq. 15), the symmetrising weights; fills the
+// cell's vectors.  Lanes of padding species (sp >= N) or absent cells contribute a = 0, w = 1.
+__device__ __forceinline__ void prepare(Core::Cell& cv, int sp, bool live, double dt, double rho_g, double rho_d,
+                                        double t_s) {
+    double a = 0.0, w = 1.0, iw = 1.0;
+    if (live) {
+        a = dt / t_s;
+        sym_weights(rho_d / rho_g, w, iw);
+    }
+    const double be = a * w;
+    const double sb = seg_sum(be * w);
+    const double amax = seg_max(a);
+    cv.a[sp] = a;
+    cv.be[sp] = be;
+    cv.w[sp] = w;
+    cv.iw[sp] = iw;
+    if (sp == 0) {
+        cv.sb = sb;
+        cv.amax = amax;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- fused a1..a5
-__global__ void __launch_bounds__(kThreads) k_update_wpc(UpdateArgs g) {
-    __shared__ WarpSmem smem[kWarps];
+__global__ void __launch_bounds__(kThreads, 2) k_update_wpc(UpdateArgs g) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpSmem& sm = smem[warp];
+    WarpSmem& sm = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
     const Core::Lane L;
     const long long nc = g.ncells;
-    const long long stride = (long long)gridDim.x * kWarps;
-    for (long long c = (long long)blockIdx.x * kWarps + warp; c < nc; c += stride) {
-        // a1: canonical lanes load their species (lane 31 doubles as the gas lane for the momenta)
-        double a = 0.0, eps = 1.0;
-        if (lane < N) {
-            a = g.dt / __ldg(g.t_s + lane * nc + c);
-            eps = __ldg(g.rho_d + lane * nc + c) / __ldg(g.rho_g + c);
-        }
-        double p[3] = {0.0, 0.0, 0.0};
-        const int k = (lane < N) ? lane + 1 : 0;  // momentum row of this lane
-        const bool has_p = (lane < N) || (lane == 31);
-        if (has_p) {
-#pragma unroll
-            for (int comp = 0; comp < 3; ++comp) p[comp] = __ldg(g.p_in + (long long)(comp * n + k) * nc + c);
-        }
-        // a2-a4
-        CellState st;
-        cell_expm(L, sm, lane, a, eps, st);
-        if (lane == 0) {
-            if (g.s_out) g.s_out[c] = st.s;
-            if (g.m_out) g.m_out[c] = st.m;
-        }
-        // a5: y = P W^-1 p_in, p_out = p_in + W y
-#pragma unroll
-        for (int comp = 0; comp < 3; ++comp) {
-            if (lane < ND) sm.q[comp][lane] = p[comp] * st.iw;  // padding lanes: p = 0
-            if (lane == 31) sm.q0[comp] = p[comp];
-        }
+    const long long ngroups = (nc + kGroup - 1) / kGroup;
+    const long long gstride = (long long)gridDim.x * kWarps;
+    const bool vec16 = (nc & 1) == 0;
+    long long grp = (long long)blockIdx.x * kWarps + warp;
+    int stage = 0;
+    request_group(g, sm.in[0], grp * kGroup, lane, vec16);
+    for (; grp < ngroups; grp += gstride, stage ^= 1) {
+        const long long c0 = grp * kGroup;
+        // the next group's rows travel while this group is worked on (an empty commit past the end keeps the
+        // wait count uniform)
+        request_group(g, sm.in[stage ^ 1], (grp + gstride) * kGroup, lane, vec16);
+        cp_async_wait<1>();
         __syncwarp();
+        double (*in)[kGroup] = sm.in[stage];
+        const int ncell = (nc - c0 < kGroup) ? (int)(nc - c0) : kGroup;
+
+        // a1 for the whole group: lane <-> (cell, species)
 #pragma unroll
-        for (int comp = 0; comp < 3; ++comp) {
-            Core::VecC qC;
-            Core::VecR yR;
-            const double q0 = sm.q0[comp];
-            double acc = 0.0;
-#pragma unroll
-            for (int I = 0; I < TL; ++I) {
-#pragma unroll
-                for (int e = 0; e < 2; ++e) qC.v[I][e] = sm.q[comp][8 * I + 2 * L.t + e];
-                acc = fma(st.rR.v[I], sm.q[comp][8 * I + L.g], acc);
+        for (int pass = 0; pass < kGroup / kPerPass; ++pass) {
+            const int k = pass * kPerPass + lane / ND, sp = lane % ND;
+            const bool live = (sp < N) && (k < ncell);
+            double rg = 1.0, rd = 1.0, ts = 1.0;
+            if (live) {
+                rg = in[0][k];
+                rd = in[1 + sp][k];
+                ts = in[1 + N + sp][k];
             }
-            Core::matvec(st.T, qC, yR);
-            const double y0 = fma(st.d0, q0, oct_sum(acc));
-#pragma unroll
-            for (int I = 0; I < TL; ++I)
-                if (L.t == 0) sm.y[comp][8 * I + L.g] = fma(st.rR.v[I], q0, yR.v[I]);
-            if (lane == 0) sm.y0[comp] = y0;
+            prepare(sm.cell[k], sp, live, g.dt, rg, rd, ts);
         }
         __syncwarp();
-        if (has_p) {
+
+        for (int k = 0; k < ncell; ++k) {
+            const Core::Cell& cv = sm.cell[k];
+            // a2-a4
+            Core::Result R;
+            Core::expm(L, cv, R);
+            if (lane == 0) {
+                if (g.s_out) g.s_out[c0 + k] = R.s;
+                if (g.m_out) g.m_out[c0 + k] = R.m;
+            }
+            // a5: y = P W^-1 p_in, p_out = p_in + W y
+            if (lane < ND) {
+                const double iw = cv.iw[lane];
+#pragma unroll
+                for (int comp = 0; comp < 3; ++comp)
+                    sm.q[comp][lane] = (lane < N) ? in[kRowsIn + comp * n + 1 + lane][k] * iw : 0.0;
+            } else if (lane < ND + 3) {
+                sm.q0[lane - ND] = in[kRowsIn + (lane - ND) * n][k];
+            }
+            __syncwarp();
 #pragma unroll
             for (int comp = 0; comp < 3; ++comp) {
-                const double y = (lane < N) ? sm.y[comp][lane] : sm.y0[comp];
-                g.p_out[(long long)(comp * n + k) * nc + c] = fma(st.w, y, p[comp]);
+                Core::VecC qC;
+                Core::VecR yR;
+                const double q0 = sm.q0[comp];
+#pragma unroll
+                for (int I = 0; I < TL; ++I)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) qC.v[I][e] = sm.q[comp][8 * I + 2 * L.t + e];
+                Core::matvec(R.T, qC, yR);
+                const double y0 = fma(R.d0, q0, Core::dotC(R.rC, qC));
+#pragma unroll
+                for (int I = 0; I < TL; ++I) {
+                    const int row = 8 * I + L.g;
+                    if (L.t == 0 && row < N) {
+                        const double y = fma(R.rR.v[I], q0, yR.v[I]);
+                        sm.out[comp * n + 1 + row][k] = fma(cv.w[row], y, in[kRowsIn + comp * n + 1 + row][k]);
+                    }
+                }
+                if (lane == 1) sm.out[comp * n][k] = q0 + y0;
+            }
+            __syncwarp();
+        }
+
+        // write the group's results: whole 32-byte sectors when aligned and complete
+        if (vec16 && ncell == kGroup) {
+            for (int it = lane; it < 2 * kRowsP; it += 32) {
+                const int r = it >> 1, h = it & 1;
+                const double2 v = *reinterpret_cast<const double2*>(&sm.out[r][2 * h]);
+                *reinterpret_cast<double2*>(g.p_out + (long long)r * nc + c0 + 2 * h) = v;
+            }
+        } else {
+            for (int it = lane; it < kGroup * kRowsP; it += 32) {
+                const int r = it >> 2, k = it & 3;
+                if (k < ncell) g.p_out[(long long)r * nc + c0 + k] = sm.out[r][k];
             }
         }
+        __syncwarp();
     }
+    cp_async_wait<0>();
 }
 
 // ---------------------------------------------------------------------------------------------- staged a2-a4
 __global__ void __launch_bounds__(kThreads) k_expm_wpc(ExpmArgs g) {
-    __shared__ WarpSmem smem[kWarps];
+    __shared__ Core::Cell cells[kWarps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpSmem& sm = smem[warp];
+    Core::Cell& cv = cells[warp];
     const Core::Lane L;
     const long long nc = g.ncells;
     const long long stride = (long long)gridDim.x * kWarps;
     for (long long c = (long long)blockIdx.x * kWarps + warp; c < nc; c += stride) {
-        double a = 0.0, eps = 1.0;
-        if (lane < N) {
-            a = __ldg(g.A + (long long)(0 * n + lane + 1) * nc + c);
-            const double b = __ldg(g.A + (long long)((lane + 1) * n + 0) * nc + c);
-            eps = a > 0.0 ? b / a : 1.0;
+        // recover a_j and eps_j from the staged matrix: A_0j = a_j, A_j0 = eps_j a_j (Eq. 17)
+        if (lane < ND) {
+            double a = 0.0, w = 1.0, iw = 1.0;
+            if (lane < N) {
+                a = __ldg(g.A + (long long)(0 * n + lane + 1) * nc + c);
+                const double b = __ldg(g.A + (long long)((lane + 1) * n + 0) * nc + c);
+                sym_weights(a > 0.0 ? b / a : 1.0, w, iw);
+            }
+            cv.a[lane] = a;
+            cv.be[lane] = a * w;
+            cv.w[lane] = w;
+            cv.iw[lane] = iw;
         }
-        CellState st;
-        cell_expm(L, sm, lane, a, eps, st);
-        if (lane == 0 && g.s_out) g.s_out[c] = st.s;
+        __syncwarp();
+        if (lane == 0) {
+            double sb = 0.0, amax = 0.0;
+            for (int j = 0; j < N; ++j) {
+                sb = fma(cv.be[j], cv.w[j], sb);
+                amax = fmax(amax, cv.a[j]);
+            }
+            cv.sb = sb;
+            cv.amax = amax;
+        }
+        __syncwarp();
+        Core::Result R;
+        Core::expm(L, cv, R);
+        if (lane == 0 && g.s_out) g.s_out[c] = R.s;
         double* E = g.E + c;
         // E = I + W P W^-1
 #pragma unroll
         for (int I = 0; I < TL; ++I) {
             const int row = 8 * I + L.g;
+            const double wr = cv.w[row];
 #pragma unroll
             for (int J = 0; J < TL; ++J)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const int col = 8 * J + 2 * L.t + e;
                     if (row < N && col < N) {
-                        const double v = (row == col) ? 1.0 + st.T[I][J][e] : st.wR.v[I] * st.T[I][J][e] * st.iwC.v[J][e];
+                        const double v = (row == col) ? 1.0 + R.T[I][J][e] : wr * R.T[I][J][e] * cv.iw[col];
                         E[(long long)((row + 1) * n + col + 1) * nc] = v;
                     }
                 }
-            if (L.t == 0 && row < N) E[(long long)((row + 1) * n) * nc] = st.wR.v[I] * st.rR.v[I];  // column 0
+            if (L.t == 0 && row < N) E[(long long)((row + 1) * n) * nc] = wr * R.rR.v[I];  // column 0
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int col = 8 * I + 2 * L.t + e;
-                if (L.g == 0 && col < N) E[(long long)(col + 1) * nc] = st.rC.v[I][e] * st.iwC.v[I][e];  // row 0
+                if (L.g == 0 && col < N) E[(long long)(col + 1) * nc] = R.rC.v[I][e] * cv.iw[col];  // row 0
             }
         }
-        if (lane == 0) E[0] = 1.0 + st.d0;
+        if (lane == 0) E[0] = 1.0 + R.d0;
         __syncwarp();
     }
 }
 
-unsigned persistent_grid(const void* kernel, long long ncells) {
+unsigned persistent_grid(const void* kernel, long long units, size_t smem) {
     int dev = 0, sms = 148, per_sm = 1;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, smem);
     if (per_sm < 1) per_sm = 1;
-    long long want = (ncells + kWarps - 1) / kWarps;
+    long long want = (units + kWarps - 1) / kWarps;
     long long cap = (long long)sms * per_sm;
     return (unsigned)(want < cap ? want : cap);
 }
 
 cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    k_update_wpc<<<persistent_grid((const void*)k_update_wpc, a.ncells), kThreads, 0, st>>>(a);
+    static bool configured[64] = {false};  // per device
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!configured[dev]) {
+        e = cudaFuncSetAttribute(k_update_wpc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        if (e != cudaSuccess) return e;
+        configured[dev] = true;
+    }
+    const long long ngroups = (a.ncells + kGroup - 1) / kGroup;
+    k_update_wpc<<<persistent_grid((const void*)k_update_wpc, ngroups, kSmemBytes), kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
 }
 cudaError_t launch_expm(const ExpmArgs& a, cudaStream_t st) {
-    k_expm_wpc<<<persistent_grid((const void*)k_expm_wpc, a.ncells), kThreads, 0, st>>>(a);
+    k_expm_wpc<<<persistent_grid((const void*)k_expm_wpc, a.ncells, 0), kThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -36,14 +36,22 @@ def run_and_compare(dg, oracle, wl, idx=None, check_s=True, variant=0):
     assert float(cons.max()) <= CONS_TOL, f"{wl.name}: conservation {float(cons.max()):.3e}"
     sv = s[idx_d].cpu().numpy(); mv = m[idx_d].cpu().numpy()
     if check_s:
-        # the (m, s) choice must satisfy Theorem 1's premise: ||A||_1 / 2^s <= theta_m (Table B.1)
+        # the (m, s) choice must satisfy Theorem 1's premise in the norm the kernels scale by
+        # (R5): ||S||_2 / 2^s <= theta_m (Table B.1), S = W^-1 (dt Omega) W the symmetrised Eq. 17, its
+        # 2-norm computed here by an eigensolver (the kernels use a closed-form upper bound)
         theta = {2: 2.5809568e-8, 4: 3.3971688e-4, 6: 9.0656564e-3, 9: 8.9577602e-2, 12: 2.9961589e-1, 16: 7.8028743e-1,
                  20: 1.4382526, 25: 2.4285825, 30: 3.5396663}
         eps = rho_d / rho_g[None, :]
         a = wl.dt / t_s
-        norm = 2.0 * np.maximum((eps * a).sum(axis=0), a.max(axis=0))
-        th = np.array([theta[int(k)] for k in mv])
-        assert (norm / 2.0 ** sv <= th * (1 + 1e-9)).all()
+        take = np.unique(np.concatenate([np.arange(0, len(sv), max(1, len(sv) // 512)), np.argsort(sv)[-16:]]))
+        S = np.zeros((len(take), wl.N + 1, wl.N + 1))
+        dust = np.arange(1, wl.N + 1)
+        S[:, 0, 0] = -(eps * a)[:, take].sum(axis=0)
+        S[:, 0, 1:] = S[:, 1:, 0] = (a * np.sqrt(eps))[:, take].T
+        S[:, dust, dust] = -a[:, take].T
+        norm2 = np.abs(np.linalg.eigvalsh(S)).max(axis=1)
+        th = np.array([theta[int(k)] for k in mv[take]])
+        assert (norm2 / 2.0 ** sv[take] <= th * (1 + 1e-9)).all()
         assert (sv >= 0).all()
     return float(err.max()), float(cons.max())
 
