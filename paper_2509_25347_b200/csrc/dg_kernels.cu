@@ -49,6 +49,8 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
     const long long nc = g.ncells;
     const long long stride = (long long)gridDim.x * kThreads;
     long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
+    long long cw = c - (threadIdx.x & 31);  // first cell of this warp: the loop is warp-uniform (the lanes take the
+                                            // Taylor degree together, dg_params.cuh); lanes past the end idle
 
     auto request_inputs = [&](long long cc) {
         if (cc < nc) {
@@ -62,22 +64,32 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
         cp_async_commit();
     };
     request_inputs(c);
-    while (c < nc) {
-        static_for<0, kRowsP>([&](auto R) {
-            constexpr int r = R;
-            cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
-        });
+    while (cw < nc) {
+        const bool valid = c < nc;
+        if (valid) {
+            static_for<0, kRowsP>([&](auto R) {
+                constexpr int r = R;
+                cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
+            });
+        }
         cp_async_commit();
         cp_async_wait<1>();  // the inputs of cell c have landed (its momenta may still be in flight)
 
-        // a1: eps_i (Eq. 14), a_i = dt alpha_i (Eq. 15), symmetrising weights
+        // a1: eps_i (Eq. 14), a_i = dt alpha_i (Eq. 15), symmetrising weights; a lane without a cell gets the
+        // identity (a = 0)
         double a[N], w[N], iw[N];
-        {
-            const double irg = 1.0 / s_in[0];
+        if (valid) {
+            const double irg = fast_rcp(s_in[0]);
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
-                a[i] = g.dt / s_in[(1 + N + i) * kThreads];
+                a[i] = g.dt * fast_rcp(s_in[(1 + N + i) * kThreads]);
                 sym_weights(s_in[(1 + i) * kThreads] * irg, w[i], iw[i]);
+            });
+        } else {
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                a[i] = 0.0;
+                w[i] = iw[i] = 1.0;
             });
         }
         const long long cn = c + stride;
@@ -87,34 +99,39 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
         double P[SZ];
         int m, s;
         Core::expm(a, w, iw, P, m, s);
-        if (g.s_out) g.s_out[c] = s;
-        if (g.m_out) g.m_out[c] = m;
+        if (valid) {
+            if (g.s_out) g.s_out[c] = s;
+            if (g.m_out) g.m_out[c] = m;
+        }
 
         // a5: p_out = p_in + W P W^-1 p_in, one component at a time
         cp_async_wait<1>();  // the momenta of cell c have landed (the next cell's inputs may still be in flight)
+        if (valid) {
 #pragma unroll 1
-        for (int comp = 0; comp < 3; ++comp) {
-            const double* pi = sp + comp * n * kThreads;
-            double* po = g.p_out + (long long)comp * n * nc + c;
-            double p[n], q[n];
-            static_for<0, n>([&](auto K) {
-                constexpr int k = K;
-                p[k] = pi[k * kThreads];
-                if constexpr (k == 0) q[k] = p[k];
-                else q[k] = p[k] * iw[k - 1];
-            });
-            static_for<0, n>([&](auto I) {
-                constexpr int i = I;
-                double y = 0.0;
+            for (int comp = 0; comp < 3; ++comp) {
+                const double* pi = sp + comp * n * kThreads;
+                double* po = g.p_out + (long long)comp * n * nc + c;
+                double p[n], q[n];
                 static_for<0, n>([&](auto K) {
                     constexpr int k = K;
-                    y = fma(P[Core::sx(i, k)], q[k], y);
+                    p[k] = pi[k * kThreads];
+                    if constexpr (k == 0) q[k] = p[k];
+                    else q[k] = p[k] * iw[k - 1];
                 });
-                if constexpr (i == 0) po[0] = p[0] + y;
-                else po[i * nc] = fma(w[i - 1], y, p[i]);
-            });
+                static_for<0, n>([&](auto I) {
+                    constexpr int i = I;
+                    double y = 0.0;
+                    static_for<0, n>([&](auto K) {
+                        constexpr int k = K;
+                        y = fma(P[Core::sx(i, k)], q[k], y);
+                    });
+                    if constexpr (i == 0) po[0] = p[0] + y;
+                    else po[i * nc] = fma(w[i - 1], y, p[i]);
+                });
+            }
         }
         c = cn;
+        cw += stride;
     }
     cp_async_wait<0>();
 }
@@ -143,20 +160,25 @@ __global__ void __launch_bounds__(kThreads) k_build(BuildArgs g) {
 // ---------------------------------------------------------------------------------------------- staged a2-a4
 __global__ void __launch_bounds__(kThreads) k_expm(ExpmArgs g) {
     const long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
-    if (c >= g.ncells) return;
+    const bool valid = c < g.ncells;  // no early return: the lanes of a warp choose the Taylor degree together
     const long long nc = g.ncells;
     const double* A = g.A + c;
     double a[N], w[N], iw[N];
 #pragma unroll
     for (int i = 1; i < n; ++i) {
-        const double ai = __ldg(A + (long long)(0 * n + i) * nc);
-        const double bi = __ldg(A + (long long)(i * n + 0) * nc);
-        a[i - 1] = ai;
-        sym_weights(ai > 0.0 ? bi / ai : 1.0, w[i - 1], iw[i - 1]);
+        a[i - 1] = 0.0;
+        w[i - 1] = iw[i - 1] = 1.0;
+        if (valid) {
+            const double ai = __ldg(A + (long long)(0 * n + i) * nc);
+            const double bi = __ldg(A + (long long)(i * n + 0) * nc);
+            a[i - 1] = ai;
+            sym_weights(ai > 0.0 ? bi * fast_rcp(ai) : 1.0, w[i - 1], iw[i - 1]);
+        }
     }
     double P[SZ];
     int m, s;
     Core::expm(a, w, iw, P, m, s);
+    if (!valid) return;
     if (g.s_out) g.s_out[c] = s;
     double* E = g.E + c;
     static_for<0, n>([&](auto I) {

@@ -39,17 +39,19 @@ __device__ __forceinline__ int scaling_exponent(double norm, double theta) {
 // with the polynomial priced by this implementation's sparse Horner recurrence, hcost = cost of one Horner step in
 // units of one squaring, instead of Pi_m dense products; reading R8).  Ties go to the lower row.
 // Non-finite norms give row 8 (m = 30).
-__device__ __forceinline__ int choose_row(double norm, float hcost) {
-    int row = kRows - 1;
-    if (!(norm <= 1.7e308)) return row;
-    float best = 3.0e38f;
-#pragma unroll
-    for (int k = 0; k < kRows; ++k) {
-        int sk = scaling_exponent(norm, c_theta[k]);
-        float cost = hcost * (float)c_m[k] + (float)sk;
-        if (cost < best) { best = cost; row = k; }
+//
+// The decision is always taken by a WHOLE, CONVERGED warp for one norm: lane k < 9 prices row k in fixed point
+// (1/256 of a squaring), one REDUX picks the minimum of (cost, row) packed into an int.  Every lane must call it.
+__device__ __forceinline__ int choose_row_warp(double norm, float hcost) {
+    const int lane = threadIdx.x & 31;
+    int packed = 0x7fffffff;
+    if (lane < kRows) {
+        const int sk = scaling_exponent(norm, c_theta[lane]);
+        const int cost = (int)(hcost * 256.0f + 0.5f) * c_m[lane] + (min(sk, 4000) << 8);
+        packed = (cost << 4) | lane;
     }
-    return row;
+    const int best = __reduce_min_sync(0xffffffffu, packed);
+    return (norm <= 1.7e308) ? (best & 15) : kRows - 1;
 }
 
 // s for a given row; a non-finite norm gives s = 0 (the NaN/Inf then propagates through the polynomial into that
@@ -59,31 +61,55 @@ __device__ __forceinline__ int s_for_row(double norm, int row) {
     return min(scaling_exponent(norm, c_theta[row]), kSMax);
 }
 
-// One cell decides alone (warp-per-cell mapping, where the whole warp holds the same norm).
+// Warp-per-cell mapping: the whole warp holds the same norm.
 __device__ __forceinline__ void choose_m_s(double norm, float hcost, int& m, int& s) {
-    const int row = choose_row(norm, hcost);
+    const int row = choose_row_warp(norm, hcost);
     m = c_m[row];
     s = s_for_row(norm, row);
 }
 
 // Thread-per-cell mapping: the lanes of a warp run the Horner loop in lock step, so a per-lane degree would cost
-// max(m) steps anyway.  The row is therefore chosen ONCE per warp, for the largest norm among the active lanes (the
-// paper rewrites Alg. 1 as the branch-reduced Alg. 2 for the same reason), and every lane then takes
-// the smallest s that satisfies Theorem 1's premise for ITS OWN norm with that row.  Any row is admissible for any
-// cell, so correctness never depends on which lanes took part.  The warp maximum is taken on the high word of the
-// double (one REDUX instruction) and rounded up: an upper bound within 2^-20, which can only cost, never break.
+// max(m) steps anyway.  The row is therefore chosen ONCE per warp, for the largest norm among its lanes (the paper
+// rewrites Alg. 1 as the branch-reduced Alg. 2 for the same reason), and every lane then takes the
+// smallest s that satisfies Theorem 1's premise for ITS OWN norm with that row.  Any row is admissible for any
+// cell, so correctness never depends on the other lanes.  The warp maximum is taken on the high word of the double
+// (one REDUX instruction) and rounded up: an upper bound within 2^-20, which can only cost, never break.
+// All 32 lanes must call it (lanes without a cell pass norm = 0).
 __device__ __forceinline__ void choose_m_s_warp(double norm, float hcost, int& m, int& s) {
-    const unsigned hi = __reduce_max_sync(__activemask(), (unsigned)__double2hiint(norm));  // NaN / Inf / negative win
+    const unsigned hi = __reduce_max_sync(0xffffffffu, (unsigned)__double2hiint(norm));  // NaN / Inf / negative win
     const double nmax = (hi >= 0x7ff00000u) ? __longlong_as_double(0x7ff0000000000000LL) : __hiloint2double((int)hi + 1, 0);
-    const int row = choose_row(nmax, hcost);
+    const int row = choose_row_warp(nmax, hcost);
     m = c_m[row];
     s = s_for_row(norm, row);
+}
+
+// 1/x and 1/sqrt(x) to about one ulp for normal positive x: the hardware seed (MUFU.RCP64H / MUFU.RSQ64H, relative
+// error < 2^-22) and two Newton steps, without the IEEE routines' exponent fix-ups and slow paths.  The drag matrix
+// takes a_i = dt/t_s,i and eps_i as DATA: an ulp of relative error in them is the same perturbation as the
+// rounding of the inputs themselves, and it keeps Eq. 17's structure (zero column sums) exactly.  Zero, subnormal,
+// infinite or NaN arguments give a non-finite result (the contract: non-finite output in that cell only); arguments
+// above 2^1022 give 0.
+__device__ __forceinline__ double fast_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+__device__ __forceinline__ double fast_rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-(x * y), y, 1.0);
+    y = fma(0.5 * y, e, y);
+    e = fma(-(x * y), y, 1.0);
+    return fma(0.5 * y, e, y);
 }
 
 // 1/sqrt(eps) and sqrt(eps) with eps clamped away from zero so that rho_d = 0 stays finite (R12).
 __device__ __forceinline__ void sym_weights(double eps, double& w, double& iw) {
     eps = fmax(eps, 1e-200);
-    iw = rsqrt(eps);
+    iw = fast_rsqrt(eps);
     w = eps * iw;
 }
 

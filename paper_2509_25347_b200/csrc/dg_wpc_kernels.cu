@@ -99,8 +99,8 @@ __device__ __forceinline__ void prepare(Core::Cell& cv, int sp, bool live, doubl
                                         double t_s) {
     double a = 0.0, w = 1.0, iw = 1.0;
     if (live) {
-        a = dt / t_s;
-        sym_weights(rho_d / rho_g, w, iw);
+        a = dt * fast_rcp(t_s);
+        sym_weights(rho_d * fast_rcp(rho_g), w, iw);
     }
     const double be = a * w;
     const double sb = seg_sum(be * w);
@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(kThreads) k_expm_wpc(ExpmArgs g) {
             if (lane < N) {
                 a = __ldg(g.A + (long long)(0 * n + lane + 1) * nc + c);
                 const double b = __ldg(g.A + (long long)((lane + 1) * n + 0) * nc + c);
-                sym_weights(a > 0.0 ? b / a : 1.0, w, iw);
+                sym_weights(a > 0.0 ? b * fast_rcp(a) : 1.0, w, iw);
             }
             cv.a[lane] = a;
             cv.be[lane] = a * w;
