@@ -62,7 +62,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(job):
         objp, src, extra = job
-        cmd = [nvcc] + NVCC_FLAGS + extra + ["-c", src, "-o", objp]
+        cmd = [nvcc] + NVCC_FLAGS + extra + os.environ.get("DG_EXTRA_FLAGS", "").split() + ["-c", src, "-o", objp]
         r = subprocess.run(cmd, capture_output=True, text=True)
         log = r.stdout + r.stderr
         with open(objp[:-2] + ".ptxas.log", "w") as f:

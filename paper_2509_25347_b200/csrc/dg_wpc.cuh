@@ -55,9 +55,11 @@ struct Wpc {
     static constexpr int n = N + 1;
     static constexpr int TL = (N <= 8) ? 1 : 2;
     static constexpr int ND = 8 * TL;
-    // fp64-pipe cycles of one Horner step over those of one squaring, as coded below (a DMMA holds the pipe for 16
-    // cycles, every other fp64 instruction for 2): prices the polynomial in choose_m_s (R8)
-    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.45f : 0.25f; }
+    // Price of one Horner step in units of one squaring for choose_m_s (R8).  By fp64-pipe cycles it is 0.25
+    // (68 vs 258; a DMMA holds the pipe for 16 cycles, any other fp64 instruction for 2), by measured time 0.45 (ncu
+    // source-level samples on config 4: the squarings run at the pipe's limit, the Horner recurrence waits on its quad
+    // reduction).  The optimum is flat between the two (102.8 / 103.6 ms at 0.25 / 0.45 on config 4).
+    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.5f : 0.3f; }
 
     struct VecR { double v[TL]; };
     struct VecC { double v[TL][2]; };
@@ -133,6 +135,59 @@ struct Wpc {
 #pragma unroll
             for (int e = 0; e < 2; ++e)
                 if (L.dg[e]) T[I][I][e] = 0.0;
+    }
+
+    // One squaring of X = [[x00, r^T], [r, D]] held as (T with its diagonal, rR/rC, x00).  Project = true re-derives
+    // the diagonal (dR, d0) from conservation and writes 1 + d back; Project = false keeps the diagonal of X X.
+    template <bool Project>
+    __device__ __forceinline__ static void square(const Lane& L, double (&T)[TL][TL][2], VecR& rR, VecC& rC,
+                                                  double& x00, const VecC& wC, const VecR& iwR, VecR& dR, double& d0) {
+        // gas row of X X: x00 r + D r
+        VecR rn;
+        matvec(T, rC, rn);
+        // dust block of X X: r r^T + D D, upper tiles by DMMA on top of the rank-one border
+        double C[TL][TL][2];
+#pragma unroll
+        for (int I = 0; I < TL; ++I)
+#pragma unroll
+            for (int J = I; J < TL; ++J) {
+                C[I][J][0] = rR.v[I] * rC.v[J][0];
+                C[I][J][1] = rR.v[I] * rC.v[J][1];
+            }
+#pragma unroll
+        for (int K = 0; K < TL; ++K)
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int I = 0; I < TL; ++I)
+#pragma unroll
+                    for (int J = I; J < TL; ++J) dmma884(C[I][J][0], C[I][J][1], T[I][K][e], T[J][K][e]);
+        if (TL == 2) {  // tile (1,0)[g][2t+e] = tile (0,1)[2t+e][g], held by lane 4 (2t+e) + g/2 in slot g & 1
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int src = 4 * (2 * L.t + e) + (L.g >> 1);
+                const double v0 = __shfl_sync(kFull, C[0][TL - 1][0], src);
+                const double v1 = __shfl_sync(kFull, C[0][TL - 1][1], src);
+                C[TL - 1][0][e] = (L.g & 1) ? v1 : v0;
+            }
+        }
+        double x00n = 0.0;
+        if (!Project) x00n = fma(x00, x00, dotC(rC, rC));  // (X X)_00 = x00^2 + r.r
+#pragma unroll
+        for (int I = 0; I < TL; ++I) {
+#pragma unroll
+            for (int J = 0; J < TL; ++J) T[I][J][0] = C[I][J][0], T[I][J][1] = C[I][J][1];
+            rR.v[I] = fma(x00, rR.v[I], rn.v[I]);
+        }
+        row_to_col(L, rR, rC);
+        if (Project) {
+            zero_diag(L, T);
+            conserve(T, rR, rC, wC, iwR, dR, d0);
+            set_diag(L, T, dR, 1.0);
+            x00 = 1.0 + d0;
+        } else {
+            x00 = x00n;
+        }
     }
 
     // What the apply step needs once P = exp(S) - I is known: the dust block T (diagonal slots = d), the gas-dust
@@ -230,48 +285,21 @@ struct Wpc {
         double d0;
         conserve(T, rR, rC, wC, iwR, dR, d0);
 
-        // s squarings of X = O + diag(1 + d)
-        for (int it = 0; it < s; ++it) {
-            set_diag(L, T, dR, 1.0);
-            const double x00 = 1.0 + d0;
-            // gas row of X X: x00 r + D r
-            VecR rn;
-            matvec(T, rC, rn);
-            // dust block of X X: r r^T + D D, upper tiles by DMMA on top of the rank-one border
-            double C[TL][TL][2];
-#pragma unroll
-            for (int I = 0; I < TL; ++I)
-#pragma unroll
-                for (int J = I; J < TL; ++J) {
-                    C[I][J][0] = rR.v[I] * rC.v[J][0];
-                    C[I][J][1] = rR.v[I] * rC.v[J][1];
-                }
-#pragma unroll
-            for (int K = 0; K < TL; ++K)
-#pragma unroll
-                for (int e = 0; e < 2; ++e)
-#pragma unroll
-                    for (int I = 0; I < TL; ++I)
-#pragma unroll
-                        for (int J = I; J < TL; ++J) dmma884(C[I][J][0], C[I][J][1], T[I][K][e], T[J][K][e]);
-            if (TL == 2) {  // tile (1,0)[g][2t+e] = tile (0,1)[2t+e][g], held by lane 4 (2t+e) + g/2 in slot g & 1
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int src = 4 * (2 * L.t + e) + (L.g >> 1);
-                    const double v0 = __shfl_sync(kFull, C[0][TL - 1][0], src);
-                    const double v1 = __shfl_sync(kFull, C[0][TL - 1][1], src);
-                    C[TL - 1][0][e] = (L.g & 1) ? v1 : v0;
-                }
-            }
-#pragma unroll
-            for (int I = 0; I < TL; ++I) {
-#pragma unroll
-                for (int J = 0; J < TL; ++J) T[I][J][0] = C[I][J][0], T[I][J][1] = C[I][J][1];
-                rR.v[I] = fma(x00, rR.v[I], rn.v[I]);
-            }
-            zero_diag(L, T);
-            row_to_col(L, rR, rC);
-            conserve(T, rR, rC, wC, iwR, dR, d0);
+        // s squarings of X = O + diag(1 + d).  The diagonal is re-derived from conservation on every OTHER squaring
+        // only (always on the last one): in between, the diagonal of X X that the DMMAs deliver anyway, a sum of
+        // squares, serves as the multiplicand.  A diagonal entry enters the off-diagonals of the next X X only as a
+        // factor (relative error ~n u), and the component of that error along the conserved mode — the one that
+        // doubles per squaring — is removed again one step later, so it never exceeds ~2 n u.
+        set_diag(L, T, dR, 1.0);
+        double x00 = 1.0 + d0;
+        int it = 0;
+        if (s & 1) {
+            square<true>(L, T, rR, rC, x00, wC, iwR, dR, d0);
+            it = 1;
+        }
+        for (; it < s; it += 2) {
+            square<false>(L, T, rR, rC, x00, wC, iwR, dR, d0);
+            square<true>(L, T, rR, rC, x00, wC, iwR, dR, d0);
         }
         set_diag(L, T, dR, 0.0);
         R.d0 = d0;

@@ -4,7 +4,8 @@
 // DRAM sector when the row is 32-byte aligned — so every byte the kernel moves is a byte the method needs (a warp
 // that loaded its single cell's fields lane by lane fetched 4-5x the algorithmic bytes, ncu round 1).  All rows of
 // the NEXT group are requested with cp.async into the warp's private double-buffered staging tile before the
-// matrix work of the current group starts; results are staged in shared memory and written back as whole sectors.
+// matrix work of the current group starts; results are staged in shared memory (over the group's own momenta rows)
+// and written back as whole sectors.
 // There is no block-level synchronisation: warps are independent, __syncwarp is the only barrier.
 #include "dg_internal.h"
 #include "dg_wpc.cuh"
@@ -30,8 +31,8 @@ constexpr int kRows = kRowsIn + kRowsP;
 constexpr int kPerPass = 32 / ND;     // cells whose species fit the 32 lanes of one prologue pass
 
 struct alignas(16) WarpSmem {
-    double in[2][kRows][kGroup];   // staged inputs, double buffered: [stage][row][cell of the group]
-    double out[kRowsP][kGroup];    // staged results
+    double in[2][kRows][kGroup];   // staged inputs, double buffered: [stage][row][cell of the group]; a cell's
+                                   // results overwrite its own momenta rows once they have been consumed
     Core::Cell cell[kGroup];       // per-cell vectors prepared by the prologue
     double q[3][ND], q0[4];        // W^-1 p_in of the current cell, per component (q0[3] pads to 16 bytes)
 };
@@ -116,7 +117,7 @@ __device__ __forceinline__ void prepare(Core::Cell& cv, int sp, bool live, doubl
 }
 
 // ---------------------------------------------------------------------------------------------- fused a1..a5
-__global__ void __launch_bounds__(kThreads, 2) k_update_wpc(UpdateArgs g) {
+__global__ void __launch_bounds__(kThreads, 3) k_update_wpc(UpdateArgs g) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem& sm = reinterpret_cast<WarpSmem*>(smem_raw)[warp];
@@ -188,10 +189,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_update_wpc(UpdateArgs g) {
                     const int row = 8 * I + L.g;
                     if (L.t == 0 && row < N) {
                         const double y = fma(R.rR.v[I], q0, yR.v[I]);
-                        sm.out[comp * n + 1 + row][k] = fma(cv.w[row], y, in[kRowsIn + comp * n + 1 + row][k]);
+                        in[kRowsIn + comp * n + 1 + row][k] = fma(cv.w[row], y, in[kRowsIn + comp * n + 1 + row][k]);
                     }
                 }
-                if (lane == 1) sm.out[comp * n][k] = q0 + y0;
+                if (lane == 1) in[kRowsIn + comp * n][k] = q0 + y0;
             }
             __syncwarp();
         }
@@ -200,13 +201,13 @@ __global__ void __launch_bounds__(kThreads, 2) k_update_wpc(UpdateArgs g) {
         if (vec16 && ncell == kGroup) {
             for (int it = lane; it < 2 * kRowsP; it += 32) {
                 const int r = it >> 1, h = it & 1;
-                const double2 v = *reinterpret_cast<const double2*>(&sm.out[r][2 * h]);
+                const double2 v = *reinterpret_cast<const double2*>(&in[kRowsIn + r][2 * h]);
                 *reinterpret_cast<double2*>(g.p_out + (long long)r * nc + c0 + 2 * h) = v;
             }
         } else {
             for (int it = lane; it < kGroup * kRowsP; it += 32) {
                 const int r = it >> 2, k = it & 3;
-                if (k < ncell) g.p_out[(long long)r * nc + c0 + k] = sm.out[r][k];
+                if (k < ncell) g.p_out[(long long)r * nc + c0 + k] = in[kRowsIn + r][k];
             }
         }
         __syncwarp();
