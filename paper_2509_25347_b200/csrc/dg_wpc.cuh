@@ -137,11 +137,25 @@ struct Wpc {
                 if (L.dg[e]) T[I][I][e] = 0.0;
     }
 
+    __device__ __forceinline__ static void load_weights(const Lane& L, const Cell& cv, VecC& wC, VecR& iwR) {
+#pragma unroll
+        for (int I = 0; I < TL; ++I) {
+            iwR.v[I] = cv.iw[8 * I + L.g];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) wC.v[I][e] = cv.w[8 * I + 2 * L.t + e];
+        }
+    }
+
     // One squaring of X = [[x00, r^T], [r, D]] held as (T with its diagonal, rR/rC, x00).  Project = true re-derives
     // the diagonal (dR, d0) from conservation and writes 1 + d back; Project = false keeps the diagonal of X X.
     template <bool Project>
-    __device__ __forceinline__ static void square(const Lane& L, double (&T)[TL][TL][2], VecR& rR, VecC& rC,
-                                                  double& x00, const VecC& wC, const VecR& iwR, VecR& dR, double& d0) {
+    __device__ __forceinline__ static void square(const Lane& L, const Cell& cv, double (&T)[TL][TL][2], VecR& rR,
+                                                  VecC& rC, double& x00, VecR& dR, double& d0) {
+        // the weights are re-read from shared memory where they are needed instead of living in registers across
+        // the DMMA phase (the kernel runs at 80 registers per thread: three blocks per SM)
+        VecC wC;
+        VecR iwR;
+        if (Project) load_weights(L, cv, wC, iwR);
         // gas row of X X: x00 r + D r
         VecR rn;
         matvec(T, rC, rn);
@@ -208,19 +222,17 @@ struct Wpc {
         const int m = R.m, s = R.s;
         const double sc = pow2neg(s);
 
-        VecR alR, beR, iwR;
-        VecC beC, wC;
+        VecR alR, beR;
+        VecC beC;
 #pragma unroll
         for (int I = 0; I < TL; ++I) {
             const int row = 8 * I + L.g;
             alR.v[I] = cv.a[row] * sc;
             beR.v[I] = cv.be[row] * sc;
-            iwR.v[I] = cv.iw[row];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int col = 8 * I + 2 * L.t + e;
                 beC.v[I][e] = cv.be[col] * sc;
-                wC.v[I][e] = cv.w[col];
             }
         }
         const double b00 = -cv.sb * sc;
@@ -283,7 +295,12 @@ struct Wpc {
         row_to_col(L, rR, rC);
         VecR dR;
         double d0;
-        conserve(T, rR, rC, wC, iwR, dR, d0);
+        {
+            VecC wC;
+            VecR iwR;
+            load_weights(L, cv, wC, iwR);
+            conserve(T, rR, rC, wC, iwR, dR, d0);
+        }
 
         // s squarings of X = O + diag(1 + d).  The diagonal is re-derived from conservation on every OTHER squaring
         // only (always on the last one): in between, the diagonal of X X that the DMMAs deliver anyway, a sum of
@@ -294,12 +311,12 @@ struct Wpc {
         double x00 = 1.0 + d0;
         int it = 0;
         if (s & 1) {
-            square<true>(L, T, rR, rC, x00, wC, iwR, dR, d0);
+            square<true>(L, cv, T, rR, rC, x00, dR, d0);
             it = 1;
         }
         for (; it < s; it += 2) {
-            square<false>(L, T, rR, rC, x00, wC, iwR, dR, d0);
-            square<true>(L, T, rR, rC, x00, wC, iwR, dR, d0);
+            square<false>(L, cv, T, rR, rC, x00, dR, d0);
+            square<true>(L, cv, T, rR, rC, x00, dR, d0);
         }
         set_diag(L, T, dR, 0.0);
         R.d0 = d0;
