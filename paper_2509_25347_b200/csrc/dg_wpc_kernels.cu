@@ -173,26 +173,52 @@ __global__ void __launch_bounds__(kThreads, 3) k_update_wpc(UpdateArgs g) {
                 sm.q0[lane - ND] = in[kRowsIn + (lane - ND) * n][k];
             }
             __syncwarp();
+            {
+                // Dust rows, all three components in ONE tensor-core product: Y = r q0^T + T Q with Q[j][comp] as the
+                // B operand (lane (g, t) supplies Q[8K + 2t + e][g], zero for g >= 3).  The accumulator hands lane
+                // (g, t) the entries Y[8I + g][2t], Y[8I + g][2t + 1]: components 0, 1 to t = 0, component 2 to t = 1,
+                // with no cross-lane reduction.
+                double Bq[TL][2];
 #pragma unroll
-            for (int comp = 0; comp < 3; ++comp) {
-                Core::VecC qC;
-                Core::VecR yR;
-                const double q0 = sm.q0[comp];
+                for (int K = 0; K < TL; ++K)
 #pragma unroll
-                for (int I = 0; I < TL; ++I)
+                    for (int e = 0; e < 2; ++e) Bq[K][e] = (L.g < 3) ? sm.q[L.g][8 * K + 2 * L.t + e] : 0.0;
+                const double q0a = (L.t < 2) ? sm.q0[2 * L.t] : 0.0;       // q0[2t]     (t = 0, 1)
+                const double q0b = (L.t == 0) ? sm.q0[1] : 0.0;             // q0[2t + 1] (t = 0)
+                double Y[TL][2];
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) qC.v[I][e] = sm.q[comp][8 * I + 2 * L.t + e];
-                Core::matvec(R.T, qC, yR);
-                const double y0 = fma(R.d0, q0, Core::dotC(R.rC, qC));
+                for (int I = 0; I < TL; ++I) {
+                    Y[I][0] = R.rR.v[I] * q0a;
+                    Y[I][1] = R.rR.v[I] * q0b;
+                }
+#pragma unroll
+                for (int K = 0; K < TL; ++K)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int I = 0; I < TL; ++I) dmma884(Y[I][0], Y[I][1], R.T[I][K][e], Bq[K][e]);
+                // gas row: y0 = d0 q0 + r . q, per component (quad reductions, independent of the product above)
+                double y0[3];
+#pragma unroll
+                for (int comp = 0; comp < 3; ++comp) {
+                    Core::VecC qC;
+#pragma unroll
+                    for (int I = 0; I < TL; ++I)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) qC.v[I][e] = sm.q[comp][8 * I + 2 * L.t + e];
+                    y0[comp] = fma(R.d0, sm.q0[comp], Core::dotC(R.rC, qC));
+                }
 #pragma unroll
                 for (int I = 0; I < TL; ++I) {
                     const int row = 8 * I + L.g;
-                    if (L.t == 0 && row < N) {
-                        const double y = fma(R.rR.v[I], q0, yR.v[I]);
-                        in[kRowsIn + comp * n + 1 + row][k] = fma(cv.w[row], y, in[kRowsIn + comp * n + 1 + row][k]);
+                    if (row < N && L.t < 2) {
+                        const double w = cv.w[row];
+                        double* slot = &in[kRowsIn + 2 * L.t * n + 1 + row][k];  // component 2t
+                        *slot = fma(w, Y[I][0], *slot);
+                        if (L.t == 0) slot[n * kGroup] = fma(w, Y[I][1], slot[n * kGroup]);  // component 1
                     }
                 }
-                if (lane == 1) in[kRowsIn + comp * n][k] = q0 + y0;
+                if (lane < 3) in[kRowsIn + lane * n][k] = sm.q0[lane] + (lane == 0 ? y0[0] : lane == 1 ? y0[1] : y0[2]);
             }
             __syncwarp();
         }
