@@ -87,6 +87,15 @@ dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const doub
                             const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                             void* stream);
 
+/* ---- M drag steps in a row: the Dustybox driver  (Sect. 3.1, Eq. 26-30) ----------------------
+ * Applies the fused update `nsteps` times with the same dt, densities and stopping times:
+ *   p_out = exp(dt Omega)^nsteps p_in, every step computed from scratch by the fused kernel, as a hydro code calls it
+ * once per time step (footnote 1).  nsteps launches on `stream`: the first reads p_in and writes
+ * p_out, the rest run in place on p_out.  p_out may alias p_in.  nsteps = 0 copies p_in to p_out.
+ * DG_EINVAL if nsteps < 0; otherwise the errors of dg_drag_update. */
+dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                               const double* p_in, int N, long long ncells, int nsteps, double* p_out, void* stream);
+
 /* Same as dg_drag_update_ex with the thread mapping forced (for measuring the mappings against each other; both
  * compute the same arithmetic and agree to rounding):
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)

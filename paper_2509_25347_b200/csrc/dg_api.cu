@@ -137,6 +137,25 @@ dg_status dg_drag_update(const double* rho_g, const double* rho_d, const double*
     return dg_drag_update_ex(rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, nullptr, nullptr, stream);
 }
 
+dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                               const double* p_in, int N, long long ncells, int nsteps, double* p_out, void* stream) {
+    if (nsteps < 0) return DG_EINVAL;
+    if (nsteps == 0) {
+        bool noop;
+        dg_status st = check_common(N, ncells, &noop);
+        if (st != DG_OK || noop) return st;
+        DG_CHECK_PTR(p_in);
+        DG_CHECK_PTR(p_out);
+        if (p_in == p_out) return DG_OK;
+        return cuda_status(cudaMemcpyAsync(p_out, p_in, sizeof(double) * 3 * (size_t)(N + 1) * (size_t)ncells,
+                                           cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+    }
+    dg_status st = dg_drag_update(rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, stream);
+    for (int k = 1; k < nsteps && st == DG_OK; ++k)
+        st = dg_drag_update(rho_g, rho_d, t_s, dt, p_out, N, ncells, p_out, stream);
+    return st;
+}
+
 int dg_launches_per_update(int N, long long ncells) {
     if (N < 1 || N > DG_NMAX || ncells <= 0) return 0;
     return 1;
