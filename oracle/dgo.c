@@ -232,5 +232,67 @@ int dgo_drag_update(const double *rho_g, const double *rho_d, const double *t_s,
     return 0;
 }
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * First-order implicit RK1 drag step (App. A.1, Eq. A.3-A.6): for a pure drag step
+ * (U^(n+1/2) = U^(n) in Eq. A.4-A.5)   U^(n+1) = (I - dt*Omega)^-1 U^(n),   i.e. solve (I - dt*Omega) q = b (Eq. A.6)
+ * for each of the three components.  The oracle is the DEFINITION: the dense matrix I - dt*Omega (Omega from
+ * dgo_cell_matrix, Eq. 17) solved by Gaussian elimination with partial pivoting in long double — the O(N^3) route of
+ * App. A.1, not the O(N) closed form of App. A.2 (Eq. A.8-A.9) that the CUDA kernel uses.
+ * Pins: tests/test_rk1.py (residual in 50-digit arithmetic, N = 1 closed form, conservation, fixed point,
+ * first-order convergence to exp(t Omega), dt -> infinity limit). */
+static int solve_dense(ld *M, ld *rhs, int n, int nrhs)   /* M n x n row-major (destroyed), rhs n x nrhs row-major */
+{
+    for (int c = 0; c < n; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < n; ++r) if (fabsl(M[r * n + c]) > fabsl(M[piv * n + c])) piv = r;
+        if (M[piv * n + c] == 0.0L) return 1;
+        if (piv != c) {
+            for (int k = 0; k < n; ++k) { ld t = M[c * n + k]; M[c * n + k] = M[piv * n + k]; M[piv * n + k] = t; }
+            for (int k = 0; k < nrhs; ++k) { ld t = rhs[c * nrhs + k]; rhs[c * nrhs + k] = rhs[piv * nrhs + k]; rhs[piv * nrhs + k] = t; }
+        }
+        for (int r = c + 1; r < n; ++r) {
+            ld f = M[r * n + c] / M[c * n + c];
+            if (f == 0.0L) continue;
+            for (int k = c; k < n; ++k) M[r * n + k] -= f * M[c * n + k];
+            for (int k = 0; k < nrhs; ++k) rhs[r * nrhs + k] -= f * rhs[c * nrhs + k];
+        }
+    }
+    for (int c = n - 1; c >= 0; --c)
+        for (int k = 0; k < nrhs; ++k) {
+            ld acc = rhs[c * nrhs + k];
+            for (int j = c + 1; j < n; ++j) acc -= M[c * n + j] * rhs[j * nrhs + k];
+            rhs[c * nrhs + k] = acc / M[c * n + c];
+        }
+    return 0;
+}
+
+int dgo_rk1_update(const double *rho_g, const double *rho_d, const double *t_s, double dt, const double *p_in,
+                   int N, long long ncells, ld *p_out, int nthreads)
+{
+    if (check_args(N, ncells)) return 1;
+    const int n = N + 1;
+    int bad = 0;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+#pragma omp parallel for schedule(static) reduction(| : bad)
+    for (long long c = 0; c < ncells; ++c) {
+        ld M[(DGO_NMAX + 1) * (DGO_NMAX + 1)], rhs[(DGO_NMAX + 1) * 3];
+        double rd[DGO_NMAX], ts[DGO_NMAX];
+        for (int i = 0; i < N; ++i) { rd[i] = rho_d[(long long)i * ncells + c]; ts[i] = t_s[(long long)i * ncells + c]; }
+        dgo_cell_matrix(rho_g[c], rd, ts, dt, N, M);                       /* M = dt*Omega          */
+        for (int k = 0; k < n * n; ++k) M[k] = -M[k];
+        for (int k = 0; k < n; ++k) M[k * n + k] += 1.0L;                  /* M = I - dt*Omega      */
+        for (int k = 0; k < n; ++k)
+            for (int comp = 0; comp < 3; ++comp) rhs[k * 3 + comp] = (ld)p_in[((long long)comp * n + k) * ncells + c];
+        bad |= solve_dense(M, rhs, n, 3);
+        for (int k = 0; k < n; ++k)
+            for (int comp = 0; comp < 3; ++comp) p_out[((long long)comp * n + k) * ncells + c] = rhs[k * 3 + comp];
+    }
+    return bad;
+}
+
 int dgo_sizeof_long_double(void) { return (int)sizeof(ld); }
 int dgo_ldbl_mant_dig(void) { return __LDBL_MANT_DIG__; }

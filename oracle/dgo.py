@@ -98,6 +98,21 @@ def drag_update(rho_g, rho_d, t_s, dt, p_in, want_E=False, nthreads=0):
     return (out, E, s) if want_E else out
 
 
+def rk1_update(rho_g, rho_d, t_s, dt, p_in, nthreads=0):
+    """First-order implicit RK1 drag step (App. A.1, Eq. A.6): p_out = (I - dt*Omega)^-1 p_in by a dense solve,
+    longdouble [3][n][ncells]."""
+    N = rho_d.shape[0]
+    rho_g, prg = _f64(rho_g); rho_d, prd = _f64(rho_d); t_s, pts = _f64(t_s); p_in, pp = _f64(p_in)
+    ncells = _shape_check(rho_g, rho_d, t_s, N)
+    n = N + 1
+    assert p_in.shape == (3, n, ncells)
+    out = np.empty((3, n, ncells), dtype=LD)
+    rc = lib().dgo_rk1_update(prg, prd, pts, C.c_double(dt), pp, C.c_int(N), C.c_longlong(ncells),
+                              out.ctypes.data_as(C.c_void_p), C.c_int(nthreads))
+    assert rc == 0
+    return out
+
+
 def parity_error(p_gpu, p_ref, p_in):
     """DESIGN.md reading R13: per cell, max_{k,comp}|p_gpu - p_ref| / max_{k,comp}|p_in|, in long double."""
     d = np.abs(np.asarray(p_gpu, dtype=LD) - np.asarray(p_ref, dtype=LD)).reshape(-1, p_ref.shape[-1]).max(axis=0)
