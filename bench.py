@@ -315,6 +315,24 @@ def run_reference(args):
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def bench_rk1(dg, wl, p_out, hbm_gbs, steps=5, warmup=3):
+    """The first-order implicit RK1 step (dg_drag_rk1, App. A.2) on the same buffers: the
+    paper's speed reference for EXP (Fig. 6-7).  Same algorithmic bytes per cell, O(N) flops: HBM roofline."""
+    for _ in range(warmup):
+        dg.dg_drag_rk1(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        dg.dg_drag_rk1(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    gbs = algorithmic_bytes_per_cell(wl.N) * wl.ncells / (ms * 1e-3) / 1e9
+    return {"ms_per_launch": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "bound": "hbm", "achieved_gbs": gbs,
+            "hbm_frac": gbs / hbm_gbs}
+
+
 def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
     p_out = torch.empty_like(wl.p_in)
     total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
@@ -329,6 +347,8 @@ def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
            "dense_products_per_cell": products, "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N),
            "mean_s": float(s.double().mean().item()), "mean_m": float(m.double().mean().item()),
            "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
+    res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs)
+    res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
     del p_out
     return res, total_ms
 

@@ -96,6 +96,14 @@ dg_status dg_drag_update_ex(const double* rho_g, const double* rho_d, const doub
 dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                const double* p_in, int N, long long ncells, int nsteps, double* p_out, void* stream);
 
+/* ---- first-order implicit RK1 drag step, O(N) closed form  (App. A.2, Eq. A.6-A.9) ----------
+ * p_out[comp] = (I - dt Omega)^-1 p_in[comp] for the three components, Omega of Eq. 17: the backward-Euler solver the
+ * paper uses as its speed reference (Fig. 6-7) and as the first-order accuracy reference (Fig. 2).  Not part of the
+ * EXP path; same buffers, layouts, aliasing rule (p_out may alias p_in) and errors as dg_drag_update.
+ * HBM traffic per cell: 8*(8N+7) bytes, O(N) flops. */
+dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
+                      int N, long long ncells, double* p_out, void* stream);
+
 /* Same as dg_drag_update_ex with the thread mapping forced (for measuring the mappings against each other; both
  * compute the same arithmetic and agree to rounding):
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)

@@ -18,7 +18,7 @@ DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
 DG_VARIANT_DEFAULT, DG_VARIANT_TPC, DG_VARIANT_WPC = range(3)
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
-           "dg_drag_update_variant", "dg_drag_update_steps",
+           "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1",
            "dg_drag_update_host", "dg_host_release", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
            "dg_status_string", "dg_last_cuda_error", "dg_version")
 
@@ -45,6 +45,7 @@ def _load():
     lib.dg_drag_update_ex.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp, vp, vp]
     lib.dg_drag_update_variant.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp, vp, i32, vp]
     lib.dg_drag_update_steps.argtypes = [vp, vp, vp, dbl, vp, i32, ll, i32, vp, vp]
+    lib.dg_drag_rk1.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
     lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
     lib.dg_host_release.argtypes = []
     lib.dg_peak_kernel.argtypes = [i32, i32, vp, ll, C.POINTER(dbl), vp]
@@ -169,6 +170,19 @@ def dg_drag_update_steps(rho_g, rho_d, t_s, dt, p_in, nsteps, p_out=None):
                                    _dev(t_s, "t_s", (N, ncells)), float(dt), _dev(p_in, "p_in", (3, n, ncells)), N,
                                    ncells, int(nsteps), _dev(p_out, "p_out", (3, n, ncells)), _stream())
     _check(st, "dg_drag_update_steps")
+    return p_out
+
+
+def dg_drag_rk1(rho_g, rho_d, t_s, dt, p_in, p_out=None):
+    """First-order implicit RK1 drag step (App. A.2, Eq. A.8-A.9): p_out = (I - dt Omega)^-1 p_in."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    st = _lib.dg_drag_rk1(_dev(rho_g, "rho_g", (ncells,)), _dev(rho_d, "rho_d", (N, ncells)),
+                          _dev(t_s, "t_s", (N, ncells)), float(dt), _dev(p_in, "p_in", (3, n, ncells)), N, ncells,
+                          _dev(p_out, "p_out", (3, n, ncells)), _stream())
+    _check(st, "dg_drag_rk1")
     return p_out
 
 

@@ -156,6 +156,22 @@ dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const d
     return st;
 }
 
+dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
+                      int N, long long ncells, double* p_out, void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
+    if (noop) return DG_OK;
+    DG_CHECK_PTR(rho_g);
+    DG_CHECK_PTR(rho_d);
+    DG_CHECK_PTR(t_s);
+    DG_CHECK_PTR(p_in);
+    DG_CHECK_PTR(p_out);
+    UpdateArgs a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, nullptr, nullptr};
+    return cuda_status(kTable[N]->rk1(a, static_cast<cudaStream_t>(stream)));
+}
+
 int dg_launches_per_update(int N, long long ncells) {
     if (N < 1 || N > DG_NMAX || ncells <= 0) return 0;
     return 1;

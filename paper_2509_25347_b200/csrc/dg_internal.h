@@ -42,6 +42,7 @@ struct Launchers {
     cudaError_t (*build)(const BuildArgs&, cudaStream_t);
     cudaError_t (*expm)(const ExpmArgs&, cudaStream_t);
     cudaError_t (*apply)(const ApplyArgs&, cudaStream_t);
+    cudaError_t (*rk1)(const UpdateArgs&, cudaStream_t);  // dg_drag_rk1 (s_out / m_out unused)
     const char* variant;
 };
 

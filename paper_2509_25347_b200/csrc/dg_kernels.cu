@@ -136,6 +136,80 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
     cp_async_wait<0>();
 }
 
+// ---------------------------------------------------------------------------------------------- RK1 (App. A.2)
+// First-order implicit drag step  U^(n+1) = (I - dt Omega)^-1 U^(n)  by the O(N) closed form of Eq. A.8-A.9
+// (PAPER.md:468-482), per component b -> q:
+//     g_i = 1 / (1 + a_i),  c_i = a_i g_i,   A = 1 + sum_i eps_i c_i,   B = sum_i c_i b_i      (a_i = dt / t_s,i)
+//     q_0 = (b_0 + B) / A,      q_i = g_i b_i + eps_i c_i q_0.
+// The paper's speed reference for the EXP solver (Fig. 6-7).  Same fields, same bytes per cell as the fused EXP
+// kernel, O(N) flops: bound by HBM.  Same persistent cp.async staging as k_update (the next cell's fields travel
+// while this cell's momenta are worked on), more blocks per SM because the state is two vectors, not two matrices.
+constexpr int kRk1MinBlocks = N <= 4 ? 6 : N <= 8 ? 4 : 2;
+
+__global__ void __launch_bounds__(kThreads, kRk1MinBlocks) k_rk1(UpdateArgs g) {
+    extern __shared__ double stage[];
+    double* s_in = stage + threadIdx.x;                      // [kRowsIn][kThreads]
+    double* sp = stage + kRowsIn * kThreads + threadIdx.x;  // [kRowsP][kThreads]
+    const long long nc = g.ncells;
+    const long long stride = (long long)gridDim.x * kThreads;
+    long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
+
+    auto request_inputs = [&](long long cc) {
+        if (cc < nc) {
+            cp_async8(s_in, g.rho_g + cc);
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                cp_async8(s_in + (1 + i) * kThreads, g.rho_d + i * nc + cc);
+                cp_async8(s_in + (1 + N + i) * kThreads, g.t_s + i * nc + cc);
+            });
+        }
+        cp_async_commit();
+    };
+    request_inputs(c);
+    while (c < nc) {
+        static_for<0, kRowsP>([&](auto R) {
+            constexpr int r = R;
+            cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
+        });
+        cp_async_commit();
+        cp_async_wait<1>();  // the fields of cell c have landed
+        double gi[N], ci[N], ei[N];
+        double A = 1.0;
+        {
+            const double irg = fast_rcp(s_in[0]);
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                const double a = g.dt * fast_rcp(s_in[(1 + N + i) * kThreads]);  // Eq. 15 times dt
+                gi[i] = fast_rcp(1.0 + a);
+                ci[i] = a * gi[i];
+                ei[i] = (s_in[(1 + i) * kThreads] * irg) * ci[i];                // eps_i c_i (Eq. 14)
+                A += ei[i];
+            });
+        }
+        const double iA = fast_rcp(A);
+        const long long cn = c + stride;
+        request_inputs(cn);
+        cp_async_wait<1>();  // the momenta of cell c have landed
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp) {
+            const double* pi = sp + comp * n * kThreads;
+            double* po = g.p_out + (long long)comp * n * nc + c;
+            double b[n];
+            static_for<0, n>([&](auto K) { b[K] = pi[K * kThreads]; });
+            double B = b[0];
+            static_for<0, N>([&](auto I) { B = fma(ci[I], b[I + 1], B); });
+            const double q0 = B * iA;
+            po[0] = q0;
+            static_for<0, N>([&](auto I) {
+                constexpr int i = I;
+                po[(i + 1) * nc] = fma(ei[i], q0, gi[i] * b[i + 1]);
+            });
+        }
+        c = cn;
+    }
+    cp_async_wait<0>();
+}
+
 // ---------------------------------------------------------------------------------------------- staged a1
 __global__ void __launch_bounds__(kThreads) k_build(BuildArgs g) {
     const long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
@@ -223,17 +297,17 @@ __global__ void __launch_bounds__(kThreads) k_apply(ApplyArgs g) {
 inline unsigned grid_for(long long ncells) { return (unsigned)((ncells + kThreads - 1) / kThreads); }
 
 // Persistent grid: as many blocks as fit on the device at once (or fewer, if there are not enough cells).
-cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    static int blocks_per_sm[64] = {0};  // per device; 0 = not yet queried
+template <class Kernel>
+cudaError_t launch_persistent(Kernel kernel, int (&blocks_per_sm)[64], const UpdateArgs& a, cudaStream_t st) {
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
     if (blocks_per_sm[dev] == 0) {
-        e = cudaFuncSetAttribute(k_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
         if (e != cudaSuccess) return e;
         int per_sm = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update, kThreads, kSmemBytes);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, kSmemBytes);
         if (e != cudaSuccess) return e;
         blocks_per_sm[dev] = per_sm > 0 ? per_sm : 1;
     }
@@ -241,8 +315,16 @@ cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     const long long want = (a.ncells + kThreads - 1) / kThreads;
     const long long cap = (long long)sms * blocks_per_sm[dev];
-    k_update<<<(unsigned)(want < cap ? want : cap), kThreads, kSmemBytes, st>>>(a);
+    kernel<<<(unsigned)(want < cap ? want : cap), kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
+}
+cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
+    static int blocks_per_sm[64] = {0};  // per device; 0 = not yet queried
+    return launch_persistent(k_update, blocks_per_sm, a, st);
+}
+cudaError_t launch_rk1(const UpdateArgs& a, cudaStream_t st) {
+    static int blocks_per_sm[64] = {0};
+    return launch_persistent(k_rk1, blocks_per_sm, a, st);
 }
 cudaError_t launch_build(const BuildArgs& a, cudaStream_t st) {
     k_build<<<grid_for(a.ncells), kThreads, 0, st>>>(a);
@@ -262,6 +344,6 @@ cudaError_t launch_apply(const ApplyArgs& a, cudaStream_t st) {
 #define DG_CAT_(a, b) a##b
 #define DG_CAT(a, b) DG_CAT_(a, b)
 extern const Launchers DG_CAT(launchers_N, DG_N) = {launch_update, launch_build, launch_expm, launch_apply,
-                                                    "thread-per-cell, symmetric packed registers"};
+                                                    launch_rk1, "thread-per-cell, symmetric packed registers"};
 
 }  // namespace dg
