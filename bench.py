@@ -333,6 +333,24 @@ def bench_rk1(dg, wl, p_out, hbm_gbs, steps=5, warmup=3):
             "hbm_frac": gbs / hbm_gbs}
 
 
+def bench_paper_variant(dg, wl, p_out, steps=2, warmup=1):
+    """The paper's own scheme as printed (DG_VARIANT_PAPER: one thread per cell, dense matrices, Alg. 7 + plain
+    squarings) on the same buffers, for the design comparison on the same hardware."""
+    f = lambda: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=dg.DG_VARIANT_PAPER)
+    for _ in range(warmup):
+        f()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        f()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    drift = ((p_out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)).max().item()
+    return {"ms_per_launch": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "max_momentum_drift": drift}
+
+
 def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
     p_out = torch.empty_like(wl.p_in)
     total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
@@ -349,6 +367,8 @@ def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
            "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
     res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs)
     res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
+    res["paper_as_printed"] = bench_paper_variant(dg, wl, p_out)
+    res["paper_as_printed"]["speedup_of_product_path"] = res["paper_as_printed"]["ms_per_launch"] / ms_launch
     del p_out
     return res, total_ms
 

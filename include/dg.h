@@ -109,10 +109,15 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)
  *   DG_VARIANT_TPC      thread-per-cell: one thread owns a cell, packed symmetric matrices in registers
  *   DG_VARIANT_WPC      warp-per-cell: one warp owns a cell, fp64 tensor-core (DMMA) tiles for the squarings
+ *   DG_VARIANT_PAPER    NOT the same arithmetic: the paper's own scheme as printed — one thread per cell, dense
+ *                       (N+1)x(N+1) fp64 matrices, Table B.1 row minimising Pi_m + s on ||A||_1 (Eq. B.11), Taylor
+ *                       polynomial by Algorithm 7, plain squarings (Alg. 6).  A measured reference for the design
+ *                       comparison; its error grows like 2^s u on stiff cells.
  * Any other value is DG_EINVAL. */
 #define DG_VARIANT_DEFAULT 0
 #define DG_VARIANT_TPC 1
 #define DG_VARIANT_WPC 2
+#define DG_VARIANT_PAPER 3
 dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                  const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                                  int variant, void* stream);

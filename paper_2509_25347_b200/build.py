@@ -2,7 +2,8 @@
 
     python -m paper_2509_25347_b200.build [--force] [--verbose]
 
-One object per translation unit, compiled in parallel: dg_kernels.cu once per species count N (-DDG_N=<N>), plus
+One object per translation unit, compiled in parallel: dg_kernels.cu, dg_wpc_kernels.cu and dg_paper_kernels.cu once
+per species count N (-DDG_N=<N>), plus
 dg_api.cu, dg_peaks.cu, dg_host.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
 nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 division, sqrt and the exponent arithmetic must stay
 IEEE.
@@ -37,6 +38,7 @@ def _units():
     for n in range(1, NMAX + 1):
         units.append((f"dg_kernels_N{n}.o", "dg_kernels.cu", [f"-DDG_N={n}"]))
         units.append((f"dg_wpc_kernels_N{n}.o", "dg_wpc_kernels.cu", [f"-DDG_N={n}"]))
+        units.append((f"dg_paper_kernels_N{n}.o", "dg_paper_kernels.cu", [f"-DDG_N={n}"]))
     return units
 
 

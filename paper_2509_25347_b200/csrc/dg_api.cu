@@ -20,6 +20,12 @@ static const WpcLaunchers* const kWpcTable[DG_NMAX + 1] = {
     &wpc_launchers_N10, &wpc_launchers_N11, &wpc_launchers_N12, &wpc_launchers_N13, &wpc_launchers_N14,
     &wpc_launchers_N15, &wpc_launchers_N16};
 
+static const PaperLaunchers* const kPaperTable[DG_NMAX + 1] = {
+    nullptr,              &paper_launchers_N1,  &paper_launchers_N2,  &paper_launchers_N3,  &paper_launchers_N4,
+    &paper_launchers_N5,  &paper_launchers_N6,  &paper_launchers_N7,  &paper_launchers_N8,  &paper_launchers_N9,
+    &paper_launchers_N10, &paper_launchers_N11, &paper_launchers_N12, &paper_launchers_N13, &paper_launchers_N14,
+    &paper_launchers_N15, &paper_launchers_N16};
+
 // The mapping dg_drag_update uses for each N, chosen from measurements on B200: registers hold the
 // packed symmetric matrices of one cell per thread up to N = 12; beyond that the thread-per-cell kernel spills and the
 // warp-per-cell DMMA kernel wins.
@@ -46,6 +52,7 @@ static dg_status check_common(int N, long long ncells, bool* noop) {
 
 cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st) {
     if (variant == DG_VARIANT_DEFAULT) variant = default_variant(N);
+    if (variant == DG_VARIANT_PAPER) return kPaperTable[N]->update(a, st);
     return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
 }
 
@@ -112,7 +119,7 @@ dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const
     dg_status st = check_common(N, ncells, &noop);
     if (st != DG_OK) return st;
     if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
-    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_WPC) return DG_EINVAL;
+    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PAPER) return DG_EINVAL;
     if (noop) return DG_OK;
     DG_CHECK_PTR(rho_g);
     DG_CHECK_PTR(rho_d);

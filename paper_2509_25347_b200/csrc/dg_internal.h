@@ -53,9 +53,16 @@ struct WpcLaunchers {
     const char* variant;
 };
 
-#define DG_DECL_LAUNCHERS(NN)                 \
-    extern const Launchers launchers_N##NN;   \
-    extern const WpcLaunchers wpc_launchers_N##NN;
+// The paper's scheme as printed (dg_paper_kernels.cu, one translation unit per N): a measured reference, not the product.
+struct PaperLaunchers {
+    cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    const char* variant;
+};
+
+#define DG_DECL_LAUNCHERS(NN)                       \
+    extern const Launchers launchers_N##NN;         \
+    extern const WpcLaunchers wpc_launchers_N##NN;  \
+    extern const PaperLaunchers paper_launchers_N##NN;
 DG_DECL_LAUNCHERS(1)
 DG_DECL_LAUNCHERS(2)
 DG_DECL_LAUNCHERS(3)
