@@ -264,11 +264,11 @@ def cpu_oracle_sample(wl, budget_s=15.0):
     from oracle import dgo
     threads = dgo.max_threads()
 
-    def run(nsample):
+    def run(nsample, nthreads=0):
         idx = W.sample_cells(wl.ncells, nsample)
         rho_g, rho_d, t_s, p_in = wl.cells(idx)
         t0 = time.perf_counter()
-        dgo.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+        dgo.drag_update(rho_g, rho_d, t_s, wl.dt, p_in, nthreads=nthreads)
         return len(idx), time.perf_counter() - t0
 
     dgo.lib()
@@ -276,8 +276,10 @@ def cpu_oracle_sample(wl, budget_s=15.0):
     rate = nc / max(sec, 1e-6)
     nsample = int(min(wl.ncells, max(2048, rate * budget_s)))
     nc, sec = run(nsample)
+    n1, sec1 = run(int(min(wl.ncells, max(1024, rate / threads * 3.0))), nthreads=1)   # ~3 s on one core
     return {"value": nc / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": f"{nc} cells strided over the {wl.ncells}-cell workload, {sec:.1f} s"}
+            "sample": f"{nc} cells strided over the {wl.ncells}-cell workload, {sec:.1f} s",
+            "value_1core": n1 / sec1, "sample_1core": f"{n1} cells, {sec1:.1f} s"}
 
 
 def run_reference(args):

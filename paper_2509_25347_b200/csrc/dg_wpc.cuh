@@ -219,7 +219,9 @@ struct Wpc {
         // ||S||_2 <= max_j a_j + sum_j eps_j a_j (dg_tpc.cuh gives the argument; R5)
         const double norm = cv.sb + cv.amax;
         choose_m_s(norm, hcost(), R.m, R.s);
-        const int m = R.m, s = R.s;
+        // every lane holds the same (m, s); passing them through REDUX puts them in uniform registers, so the compiler
+        // knows the Horner and squaring loops are warp-uniform and drops the divergence guards around their shuffles
+        const int m = __reduce_max_sync(kFull, R.m), s = __reduce_max_sync(kFull, R.s);
         const double sc = pow2neg(s);
 
         VecR alR, beR;
