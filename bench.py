@@ -68,11 +68,11 @@ def useful_flops(N, s, m):
     n = N + 1
     tri = n * (n - 1) // 2                       # strict upper triangle
     build = (1 + 2 * N) + 3 * N + (3 * N + 2)    # 1/rho_g, dt/t_s, eps; rsqrt, w; norm (N fma + max) and scaling
-    first = 2 * N + 2 + N                        # al, be, b00 and P = B/m (row 0 only)
-    horner = ((2 * N + 1)                        # B_j = B/j: alpha, beta, b00 scaled
+    first = 4 * N + tri                          # al, be (mul), b00 (N fma); P = Q_1/m! on the strict upper triangle
+    horner = (1                                  # kappa_j = m!/j!
               + (N * (N - 1) // 2) * 3           # dust block off the diagonal, packed: mul + fma per entry
-              + (2 * N - 1)                      # (B_j P)_00: one mul + (N-1) fma
-              + 1 + 3 * N + 2)                   # 1 + P_00; row 0 from column 0 (mul + fma each); P_00
+              + (2 * N - 1)                      # (B Q)_00: one mul + (N-1) fma
+              + 1 + 3 * N + 2)                   # kappa_j + Q_00; row 0 from column 0 (mul + fma each); Q_00
     conserve = (2 * N + 1) + N * (1 + 2 * (N - 1) + 1)
     square = n + tri * (1 + 2 * N) + conserve    # 1 + d; offdiag(X X): mul + N fma per entry; diagonal from conservation
     apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)

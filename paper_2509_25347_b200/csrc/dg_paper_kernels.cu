@@ -34,16 +34,6 @@ constexpr int kUnroll = (n <= 9) ? n : 1;
 
 __constant__ const int c_q[kRows] = {1, 2, 2, 3, 3, 4, 4, 5, 5};  // Table B.1: m_k = q_k r_k
 __constant__ const int c_r[kRows] = {2, 2, 3, 3, 4, 4, 5, 5, 6};
-__constant__ const double c_ifact[31] = {  // b_i = 1/i!
-    1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880, 1.0 / 3628800,
-    1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0, 1.0 / 87178291200.0, 1.0 / 1307674368000.0,
-    1.0 / 20922789888000.0, 1.0 / 355687428096000.0, 1.0 / 6402373705728000.0, 1.0 / 121645100408832000.0,
-    1.0 / 2432902008176640000.0, 1.0 / 51090942171709440000.0, 1.0 / 1124000727777607680000.0,
-    1.0 / 25852016738884976640000.0, 1.0 / 620448401733239439360000.0, 1.0 / 15511210043330985984000000.0,
-    1.0 / 403291461126605635584000000.0, 1.0 / 10888869450418352160768000000.0,
-    1.0 / 304888344611713860501504000000.0, 1.0 / 8841761993739701954543616000000.0,
-    1.0 / 265252859812191058636308480000000.0};
-
 // Z = X Y, dense, row-major
 __device__ __forceinline__ void matmul(const double (&X)[NN], const double (&Y)[NN], double (&Z)[NN]) {
 #pragma unroll kUnroll

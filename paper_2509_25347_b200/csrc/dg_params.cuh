@@ -14,12 +14,19 @@ __constant__ const int c_m[kRows] = {2, 4, 6, 9, 12, 16, 20, 25, 30};
 __constant__ const double c_theta[kRows] = {2.5809568029e-8, 3.3971688399e-4, 9.0656564075e-3,
                                             8.9577602032e-2, 2.9961589138e-1, 7.8028742566e-1,
                                             1.4382525967,    2.4285825244,    3.5396663487};
-// 1/j for the Horner recurrence P <- (B + B P)/j, j = 1..30 (index 0 unused)
-__constant__ const double c_inv[31] = {
-    0.0,        1.0 / 1.0,  1.0 / 2.0,  1.0 / 3.0,  1.0 / 4.0,  1.0 / 5.0,  1.0 / 6.0,  1.0 / 7.0,
-    1.0 / 8.0,  1.0 / 9.0,  1.0 / 10.0, 1.0 / 11.0, 1.0 / 12.0, 1.0 / 13.0, 1.0 / 14.0, 1.0 / 15.0,
-    1.0 / 16.0, 1.0 / 17.0, 1.0 / 18.0, 1.0 / 19.0, 1.0 / 20.0, 1.0 / 21.0, 1.0 / 22.0, 1.0 / 23.0,
-    1.0 / 24.0, 1.0 / 25.0, 1.0 / 26.0, 1.0 / 27.0, 1.0 / 28.0, 1.0 / 29.0, 1.0 / 30.0};
+// 1/i!, i = 0..30: the Taylor coefficients b_i of Eq. 19
+__constant__ const double c_ifact[31] = {
+    1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320, 1.0 / 362880, 1.0 / 3628800,
+    1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0, 1.0 / 87178291200.0, 1.0 / 1307674368000.0,
+    1.0 / 20922789888000.0, 1.0 / 355687428096000.0, 1.0 / 6402373705728000.0, 1.0 / 121645100408832000.0,
+    1.0 / 2432902008176640000.0, 1.0 / 51090942171709440000.0, 1.0 / 1124000727777607680000.0,
+    1.0 / 25852016738884976640000.0, 1.0 / 620448401733239439360000.0, 1.0 / 15511210043330985984000000.0,
+    1.0 / 403291461126605635584000000.0, 1.0 / 10888869450418352160768000000.0,
+    1.0 / 304888344611713860501504000000.0, 1.0 / 8841761993739701954543616000000.0,
+    1.0 / 265252859812191058636308480000000.0};
+// j as a double, j = 0..30 (the running factor m!/j! of the unscaled Horner recurrence)
+__constant__ const double c_dbl[31] = {0,  1,  2,  3,  4,  5,  6,  7,  8,  9,  10, 11, 12, 13, 14, 15,
+                                       16, 17, 18, 19, 20, 21, 22, 23, 24, 25, 26, 27, 28, 29, 30};
 
 constexpr int kSMax = 1000;  // 2^-s must stay a normal double
 

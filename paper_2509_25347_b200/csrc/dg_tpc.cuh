@@ -12,7 +12,7 @@
 //     - Taylor polynomial (Eq. 19) without ever adding I:   P <- B_j + B_j P,  B_j = B / j,  j = m .. 1,
 //       B = S / 2^s.  B has 3N+1 non-zeros, and P is a polynomial in B, so B P = P B is symmetric: row 0 of B P is
 //       its column 0, (B P)_0k = (B P)_k0 = beta_k P_00 - alpha_k P_0k, and only (B P)_00 needs a dot product.  One
-//       Horner step is N^2 + 4N + 3 fp64-pipe instructions.
+//       Horner step is N^2 + 2N + 3 fp64-pipe instructions (the recurrence is carried unscaled, see expm()).
 //     - Squaring (Eq. 23-24):  O <- offdiag((O + diag(1+d))^2), a sum of non-negative products,
 //       so the s squarings amplify no cancellation error and total momentum is conserved to rounding at every step.
 //   * Apply (Eq. 18):  p_out = p_in + W P W^-1 p_in.
@@ -48,7 +48,7 @@ struct Tpc {
 
     // fp64-pipe instructions of one Horner step and of one squaring (with its conservation sums) as coded below;
     // their ratio prices the polynomial in choose_m_s (R8).
-    static constexpr int kHornerOps = N * N + 4 * N + 3;
+    static constexpr int kHornerOps = N * N + 2 * N + 3;
     static constexpr int kSquareOps = n * n * (n - 1) / 2 + n * n + n;
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
@@ -98,48 +98,52 @@ struct Tpc {
         });
         b00 = -b00;
 
-        // P = B / m
-        {
-            const double r = c_inv[m];
-            static_for<0, SZ>([&](auto K) { P[K] = 0.0; });
-            P[ix(0, 0)] = b00 * r;
-            static_for<1, n>([&](auto I) {
-                constexpr int i = I;
-                P[ix(0, i)] = be[i - 1] * r;
-            });
-        }
-        // P <- B_j + B_j P,  B_j = B / j.  Every right-hand side below uses the OLD row 0 of P.
+        // Q_m = B.  The recurrence runs on Q_j = (m!/j!) P_j, for which  P_j = (B + B P_{j+1}) / j  reads
+        //     Q_j = kappa_j B + B Q_{j+1},   kappa_j = m!/j!,
+        // so B is never rescaled per step (2N+1 multiplications saved per step); P = Q_1 / m! at the end.
+        static_for<0, SZ>([&](auto K) { P[K] = 0.0; });
+        P[ix(0, 0)] = b00;
+        static_for<1, n>([&](auto I) {
+            constexpr int i = I;
+            P[ix(0, i)] = be[i - 1];
+        });
+        double kap = 1.0;
+        // Every right-hand side below uses the OLD row 0 of Q.
         for (int j = m - 1; j >= 1; --j) {
-            const double r = c_inv[j];
-            double alj[N], bej[N];
-            static_for<0, N>([&](auto I) {
-                constexpr int i = I;
-                alj[i] = al[i] * r;
-                bej[i] = be[i] * r;
-            });
-            // dust block, i >= 1, off the diagonal: (B_j P)_ik = beta_i P_0k - alpha_i P_ik.  The dust DIAGONAL is not
+            kap *= c_dbl[j + 1];
+            // dust block, i >= 1, off the diagonal: (B Q)_ik = beta_i Q_0k - alpha_i Q_ik.  The dust DIAGONAL is not
             // carried through the polynomial at all: a Horner step feeds P_ii only back into P_ii, and the final
             // diagonal is re-derived from conservation below.
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
                 static_for<i + 1, n>([&](auto K) {
                     constexpr int k = K;
-                    P[ix(i, k)] = fma(bej[i - 1], P[ix(0, k)], -alj[i - 1] * P[ix(i, k)]);
+                    P[ix(i, k)] = fma(be[i - 1], P[ix(0, k)], -al[i - 1] * P[ix(i, k)]);
                 });
             });
-            // (B_j P)_00 = b00_j P_00 + sum_l beta_l P_l0
-            double t00 = bej[0] * P[ix(0, 1)];
+            // (B Q)_00 = b00 Q_00 + sum_l beta_l Q_l0
+            double t00 = be[0] * P[ix(0, 1)];
             static_for<2, n>([&](auto L) {
                 constexpr int l = L;
-                t00 = fma(bej[l - 1], P[ix(0, l)], t00);
+                t00 = fma(be[l - 1], P[ix(0, l)], t00);
             });
-            // row 0, k >= 1, from column 0 of the symmetric product: beta_k P_00 - alpha_k P_0k, plus B_j's beta_k
-            const double x00 = 1.0 + P[ix(0, 0)];
+            // row 0, k >= 1, from column 0 of the symmetric product: beta_k Q_00 - alpha_k Q_0k, plus kappa_j beta_k
+            const double x00 = kap + P[ix(0, 0)];
             static_for<1, n>([&](auto K) {
                 constexpr int k = K;
-                P[ix(0, k)] = fma(bej[k - 1], x00, -alj[k - 1] * P[ix(0, k)]);
+                P[ix(0, k)] = fma(be[k - 1], x00, -al[k - 1] * P[ix(0, k)]);
             });
-            P[ix(0, 0)] = fma(b00 * r, x00, t00);
+            P[ix(0, 0)] = fma(b00, x00, t00);
+        }
+        {
+            const double inv = c_ifact[m];  // P = Q_1 / m!
+            static_for<0, n>([&](auto I) {
+                constexpr int i = I;
+                static_for<i + 1, n>([&](auto K) {
+                    constexpr int k = K;
+                    P[ix(i, k)] *= inv;
+                });
+            });
         }
         // off-diagonals are non-negative in exact arithmetic; clamp the rounding noise, then re-derive the diagonal
         static_for<0, n>([&](auto I) {

@@ -242,57 +242,53 @@ struct Wpc {
         VecR& rR = R.rR;
         VecC& rC = R.rC;
 
-        // P = B / m.  The dust diagonal of P is never carried through the polynomial: a Horner step feeds P_ii only
-        // back into P_ii, and the final diagonal is re-derived from conservation anyway; the diagonal slots of T hold
-        // bounded don't-care values until zero_diag() below.
-        double p00;
-        {
-            const double r = c_inv[m];
+        // Q_m = B, then Q_j = kappa_j B + B Q_{j+1} with kappa_j = m!/j! (the unscaled form of P <- (B + B P)/j, see
+        // dg_tpc.cuh), P = Q_1 / m!.  (B Q)_0k is taken from column 0 of the symmetric product.  The dust diagonal is
+        // never carried through the polynomial: a Horner step feeds P_ii only back into P_ii, and the final diagonal
+        // is re-derived from conservation anyway; the diagonal slots of T hold bounded don't-care values until
+        // zero_diag() below.
+        double p00 = b00;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) {
+        for (int I = 0; I < TL; ++I) {
 #pragma unroll
-                for (int J = 0; J < TL; ++J) T[I][J][0] = T[I][J][1] = 0.0;
-                rR.v[I] = beR.v[I] * r;
-            }
-#pragma unroll
-            for (int J = 0; J < TL; ++J)
-#pragma unroll
-                for (int e = 0; e < 2; ++e) rC.v[J][e] = beC.v[J][e] * r;
-            p00 = b00 * r;
+            for (int J = 0; J < TL; ++J) T[I][J][0] = T[I][J][1] = 0.0;
+            rR.v[I] = beR.v[I];
         }
-        // P <- (B + B P) / j, with (B P)_0k taken from column 0 of the symmetric product (dg_tpc.cuh)
-        for (int j = m - 1; j >= 1; --j) {
-            const double r = c_inv[j];
-            VecR aj, bj;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) {
-                aj.v[I] = alR.v[I] * r;
-                bj.v[I] = beR.v[I] * r;
-            }
-            // dust block: (B_j P)_ik = beta_i P_0k - alpha_i P_ik
+        for (int J = 0; J < TL; ++J)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) rC.v[J][e] = beC.v[J][e];
+        double kap = 1.0;
+        for (int j = m - 1; j >= 1; --j) {
+            kap *= c_dbl[j + 1];
+            // dust block: (B Q)_ik = beta_i Q_0k - alpha_i Q_ik
 #pragma unroll
             for (int I = 0; I < TL; ++I)
 #pragma unroll
                 for (int J = 0; J < TL; ++J)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) T[I][J][e] = fma(bj.v[I], rC.v[J][e], -aj.v[I] * T[I][J][e]);
-            // (B_j P)_00 = b00_j P_00 + sum_l beta_l P_l0 ;  row 0: beta_k (1 + P_00) - alpha_k P_0k  (old values)
-            const double t00 = dotC(beC, rC) * r;
-            const double x00 = 1.0 + p00;
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = fma(beR.v[I], rC.v[J][e], -alR.v[I] * T[I][J][e]);
+            // (B Q)_00 = b00 Q_00 + sum_l beta_l Q_l0 ;  row 0: beta_k (kappa_j + Q_00) - alpha_k Q_0k  (old values)
+            const double t00 = dotC(beC, rC);
+            const double x00 = kap + p00;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) rR.v[I] = fma(bj.v[I], x00, -aj.v[I] * rR.v[I]);
+            for (int I = 0; I < TL; ++I) rR.v[I] = fma(beR.v[I], x00, -alR.v[I] * rR.v[I]);
             row_to_col(L, rR, rC);
-            p00 = fma(b00 * r, x00, t00);
+            p00 = fma(b00, x00, t00);
         }
-        // clamp the off-diagonals (non-negative in exact arithmetic), re-derive the diagonal from conservation
+        // P = Q_1 / m!; clamp the off-diagonals (non-negative in exact arithmetic), re-derive the diagonal from
+        // conservation
         zero_diag(L, T);
+        {
+            const double inv = c_ifact[m];
 #pragma unroll
-        for (int I = 0; I < TL; ++I) {
+            for (int I = 0; I < TL; ++I) {
 #pragma unroll
-            for (int J = 0; J < TL; ++J)
+                for (int J = 0; J < TL; ++J)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) T[I][J][e] = fmax(T[I][J][e], 0.0);
-            rR.v[I] = fmax(rR.v[I], 0.0);
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = fmax(T[I][J][e] * inv, 0.0);
+                rR.v[I] = fmax(rR.v[I] * inv, 0.0);
+            }
         }
         row_to_col(L, rR, rC);
         VecR dR;
