@@ -68,11 +68,11 @@ def useful_flops(N, s, m):
     n = N + 1
     tri = n * (n - 1) // 2                       # strict upper triangle
     build = (1 + 2 * N) + 3 * N + (3 * N + 2)    # 1/rho_g, dt/t_s, eps; rsqrt, w; norm (N fma + max) and scaling
-    first = 4 * N + tri                          # al, be (mul), b00 (N fma); P = Q_1/m! on the strict upper triangle
+    first = 5 * N + (N * N + N)                  # al, be, be^2 (mul), b00 (N fma); P = (beta beta^T o U, beta o v) / m!
     horner = (1                                  # kappa_j = m!/j!
-              + (N * (N - 1) // 2) * 3           # dust block off the diagonal, packed: mul + fma per entry
-              + (2 * N - 1)                      # (B Q)_00: one mul + (N-1) fma
-              + 1 + 3 * N + 2)                   # kappa_j + Q_00; row 0 from column 0 (mul + fma each); Q_00
+              + N * (N - 1)                      # U_ik <- v_k - alpha_i U_ik: one fma per packed dust entry
+              + (2 * N - 1)                      # sum_l beta_l^2 v_l: one mul + (N-1) fma
+              + 1 + 2 * N + 2)                   # kappa_j + Q_00; v_k <- x00 - alpha_k v_k (fma each); Q_00 (fma)
     conserve = (2 * N + 1) + N * (1 + 2 * (N - 1) + 1)
     square = n + tri * (1 + 2 * N) + conserve    # 1 + d; offdiag(X X): mul + N fma per entry; diagonal from conservation
     apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)

@@ -12,7 +12,7 @@
 //     - Taylor polynomial (Eq. 19) without ever adding I:   P <- B_j + B_j P,  B_j = B / j,  j = m .. 1,
 //       B = S / 2^s.  B has 3N+1 non-zeros, and P is a polynomial in B, so B P = P B is symmetric: row 0 of B P is
 //       its column 0, (B P)_0k = (B P)_k0 = beta_k P_00 - alpha_k P_0k, and only (B P)_00 needs a dot product.  One
-//       Horner step is N^2 + 2N + 3 fp64-pipe instructions (the recurrence is carried unscaled, see expm()).
+//       Horner step is N(N-1)/2 + 2N + 3 fp64-pipe instructions (see expm() for the two further rewritings).
 //     - Squaring (Eq. 23-24):  O <- offdiag((O + diag(1+d))^2), a sum of non-negative products,
 //       so the s squarings amplify no cancellation error and total momentum is conserved to rounding at every step.
 //   * Apply (Eq. 18):  p_out = p_in + W P W^-1 p_in.
@@ -48,7 +48,7 @@ struct Tpc {
 
     // fp64-pipe instructions of one Horner step and of one squaring (with its conservation sums) as coded below;
     // their ratio prices the polynomial in choose_m_s (R8).
-    static constexpr int kHornerOps = N * N + 2 * N + 3;
+    static constexpr int kHornerOps = N * (N - 1) / 2 + 2 * N + 3;
     static constexpr int kSquareOps = n * n * (n - 1) / 2 + n * n + n;
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
@@ -98,50 +98,57 @@ struct Tpc {
         });
         b00 = -b00;
 
-        // Q_m = B.  The recurrence runs on Q_j = (m!/j!) P_j, for which  P_j = (B + B P_{j+1}) / j  reads
-        //     Q_j = kappa_j B + B Q_{j+1},   kappa_j = m!/j!,
-        // so B is never rescaled per step (2N+1 multiplications saved per step); P = Q_1 / m! at the end.
+        // The polynomial.  Three rewritings of Horner's  P_j = (B + B P_{j+1}) / j  make a step N(N-1)/2 + 2N + 3 fused
+        // multiply-adds and nothing else:
+        //  (i)   Q_j = (m!/j!) P_j satisfies  Q_j = kappa_j B + B Q_{j+1},  kappa_j = m!/j!  — B is never rescaled;
+        //  (ii)  Q_j is a polynomial in B, so B Q = Q B is symmetric: its row 0 is its column 0,
+        //        (B Q)_0k = beta_k Q_00 - alpha_k Q_0k, and the dust block is (B Q)_ik = beta_i Q_0k - alpha_i Q_ik;
+        //  (iii) every entry of Q outside (0,0) carries its beta's as plain factors, Q_0k = beta_k v_k and
+        //        Q_ik = beta_i beta_k U_ik, and in (v, U) the recurrences lose their multiplications:
+        //            U_ik <- v_k - alpha_i U_ik,   v_k <- (kappa_j + Q_00) - alpha_k v_k,
+        //            Q_00 <- b00 (kappa_j + Q_00) + sum_l beta_l^2 v_l        (all right-hand sides: OLD values).
+        //        No division is ever performed (Q_m = B is v = 1, U = 0), so beta_k = 0 needs no special case.
+        // The dust DIAGONAL is not carried at all: a step feeds P_ii only back into P_ii, and the final diagonal is
+        // re-derived from conservation below.  P = Q_1 / m! is put back together at the end.
+        // Storage: P[ix(0,k)] holds v_k, P[ix(i,k)] (1 <= i < k) holds U_ik, P[ix(0,0)] holds Q_00.
+        double be2[N];
+        static_for<0, N>([&](auto I) { be2[I] = be[I] * be[I]; });
         static_for<0, SZ>([&](auto K) { P[K] = 0.0; });
         P[ix(0, 0)] = b00;
-        static_for<1, n>([&](auto I) {
-            constexpr int i = I;
-            P[ix(0, i)] = be[i - 1];
-        });
+        static_for<1, n>([&](auto I) { P[ix(0, I)] = 1.0; });
         double kap = 1.0;
-        // Every right-hand side below uses the OLD row 0 of Q.
         for (int j = m - 1; j >= 1; --j) {
             kap *= c_dbl[j + 1];
-            // dust block, i >= 1, off the diagonal: (B Q)_ik = beta_i Q_0k - alpha_i Q_ik.  The dust DIAGONAL is not
-            // carried through the polynomial at all: a Horner step feeds P_ii only back into P_ii, and the final
-            // diagonal is re-derived from conservation below.
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
                 static_for<i + 1, n>([&](auto K) {
                     constexpr int k = K;
-                    P[ix(i, k)] = fma(be[i - 1], P[ix(0, k)], -al[i - 1] * P[ix(i, k)]);
+                    P[ix(i, k)] = fma(-al[i - 1], P[ix(i, k)], P[ix(0, k)]);
                 });
             });
-            // (B Q)_00 = b00 Q_00 + sum_l beta_l Q_l0
-            double t00 = be[0] * P[ix(0, 1)];
+            double t00 = be2[0] * P[ix(0, 1)];
             static_for<2, n>([&](auto L) {
                 constexpr int l = L;
-                t00 = fma(be[l - 1], P[ix(0, l)], t00);
+                t00 = fma(be2[l - 1], P[ix(0, l)], t00);
             });
-            // row 0, k >= 1, from column 0 of the symmetric product: beta_k Q_00 - alpha_k Q_0k, plus kappa_j beta_k
             const double x00 = kap + P[ix(0, 0)];
             static_for<1, n>([&](auto K) {
                 constexpr int k = K;
-                P[ix(0, k)] = fma(be[k - 1], x00, -al[k - 1] * P[ix(0, k)]);
+                P[ix(0, k)] = fma(-al[k - 1], P[ix(0, k)], x00);
             });
             P[ix(0, 0)] = fma(b00, x00, t00);
         }
         {
-            const double inv = c_ifact[m];  // P = Q_1 / m!
-            static_for<0, n>([&](auto I) {
+            // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!
+            const double inv = c_ifact[m];
+            double bs[N];
+            static_for<0, N>([&](auto I) { bs[I] = be[I] * inv; });
+            static_for<1, n>([&](auto I) {
                 constexpr int i = I;
+                P[ix(0, i)] *= bs[i - 1];
                 static_for<i + 1, n>([&](auto K) {
                     constexpr int k = K;
-                    P[ix(i, k)] *= inv;
+                    P[ix(i, k)] *= bs[i - 1] * be[k - 1];
                 });
             });
         }

@@ -55,11 +55,10 @@ struct Wpc {
     static constexpr int n = N + 1;
     static constexpr int TL = (N <= 8) ? 1 : 2;
     static constexpr int ND = 8 * TL;
-    // Price of one Horner step in units of one squaring for choose_m_s (R8).  By fp64-pipe cycles it is 0.25
-    // (68 vs 258; a DMMA holds the pipe for 16 cycles, any other fp64 instruction for 2), by measured time 0.45 (ncu
-    // source-level samples on config 4: the squarings run at the pipe's limit, the Horner recurrence waits on its quad
-    // reduction).  The optimum is flat between the two (102.8 / 103.6 ms at 0.25 / 0.45 on config 4).
-    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.5f : 0.3f; }
+    // Price of one Horner step in units of one squaring for choose_m_s (R8): about 23 fp64 instructions
+    // and one quad reduction against 12 DMMA (16 pipe cycles each) + ~33 fp64 instructions + 32 SHFL for a squaring.
+    // The optimum is flat (config 4 timed within 1 % for prices between 0.2 and 0.45).
+    __host__ __device__ static constexpr float hcost() { return TL == 1 ? 0.4f : 0.22f; }
 
     struct VecR { double v[TL]; };
     struct VecC { double v[TL][2]; };
@@ -242,52 +241,59 @@ struct Wpc {
         VecR& rR = R.rR;
         VecC& rC = R.rC;
 
-        // Q_m = B, then Q_j = kappa_j B + B Q_{j+1} with kappa_j = m!/j! (the unscaled form of P <- (B + B P)/j, see
-        // dg_tpc.cuh), P = Q_1 / m!.  (B Q)_0k is taken from column 0 of the symmetric product.  The dust diagonal is
-        // never carried through the polynomial: a Horner step feeds P_ii only back into P_ii, and the final diagonal
-        // is re-derived from conservation anyway; the diagonal slots of T hold bounded don't-care values until
-        // zero_diag() below.
-        double p00 = b00;
+        // The polynomial, in the factored unscaled form of dg_tpc.cuh: Q_j = (m!/j!) P_j with Q_0k = beta_k v_k and
+        // Q_ik = beta_i beta_k U_ik, so that one Horner step is
+        //     U_ik <- v_k - alpha_i U_ik,   v_k <- (kappa_j + Q_00) - alpha_k v_k,
+        //     Q_00 <- b00 (kappa_j + Q_00) + sum_l beta_l^2 v_l          (right-hand sides: OLD values),
+        // one fused multiply-add per entry.  T holds U during the loop; v is carried in both replicated forms (vR,
+        // vC) elementwise, so the only cross-lane traffic of a step is the quad reduction of the sum.  The dust
+        // diagonal is never carried: the diagonal slots of T hold bounded don't-care values until zero_diag() below.
+        VecC alC, be2C, vC;
+        VecR vR;
 #pragma unroll
         for (int I = 0; I < TL; ++I) {
 #pragma unroll
             for (int J = 0; J < TL; ++J) T[I][J][0] = T[I][J][1] = 0.0;
-            rR.v[I] = beR.v[I];
+            vR.v[I] = 1.0;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                alC.v[I][e] = cv.a[8 * I + 2 * L.t + e] * sc;
+                be2C.v[I][e] = beC.v[I][e] * beC.v[I][e];
+                vC.v[I][e] = 1.0;
+            }
         }
-#pragma unroll
-        for (int J = 0; J < TL; ++J)
-#pragma unroll
-            for (int e = 0; e < 2; ++e) rC.v[J][e] = beC.v[J][e];
-        double kap = 1.0;
+        double p00 = b00, kap = 1.0;
         for (int j = m - 1; j >= 1; --j) {
             kap *= c_dbl[j + 1];
-            // dust block: (B Q)_ik = beta_i Q_0k - alpha_i Q_ik
 #pragma unroll
             for (int I = 0; I < TL; ++I)
 #pragma unroll
                 for (int J = 0; J < TL; ++J)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) T[I][J][e] = fma(beR.v[I], rC.v[J][e], -alR.v[I] * T[I][J][e]);
-            // (B Q)_00 = b00 Q_00 + sum_l beta_l Q_l0 ;  row 0: beta_k (kappa_j + Q_00) - alpha_k Q_0k  (old values)
-            const double t00 = dotC(beC, rC);
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = fma(-alR.v[I], T[I][J][e], vC.v[J][e]);
+            const double t00 = dotC(be2C, vC);
             const double x00 = kap + p00;
 #pragma unroll
-            for (int I = 0; I < TL; ++I) rR.v[I] = fma(beR.v[I], x00, -alR.v[I] * rR.v[I]);
-            row_to_col(L, rR, rC);
+            for (int I = 0; I < TL; ++I) {
+                vR.v[I] = fma(-alR.v[I], vR.v[I], x00);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) vC.v[I][e] = fma(-alC.v[I][e], vC.v[I][e], x00);
+            }
             p00 = fma(b00, x00, t00);
         }
-        // P = Q_1 / m!; clamp the off-diagonals (non-negative in exact arithmetic), re-derive the diagonal from
-        // conservation
+        // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!; clamp the off-diagonals (non-negative in exact
+        // arithmetic), re-derive the diagonal from conservation
         zero_diag(L, T);
         {
             const double inv = c_ifact[m];
 #pragma unroll
             for (int I = 0; I < TL; ++I) {
+                const double bs = beR.v[I] * inv;
 #pragma unroll
                 for (int J = 0; J < TL; ++J)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) T[I][J][e] = fmax(T[I][J][e] * inv, 0.0);
-                rR.v[I] = fmax(rR.v[I] * inv, 0.0);
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = fmax(T[I][J][e] * (bs * beC.v[J][e]), 0.0);
+                rR.v[I] = fmax(bs * vR.v[I], 0.0);
             }
         }
         row_to_col(L, rR, rC);
