@@ -52,13 +52,18 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
     long long cw = c - (threadIdx.x & 31);  // first cell of this warp: the loop is warp-uniform (the lanes take the
                                             // Taylor degree together, dg_params.cuh); lanes past the end idle
 
+    // row addresses by running pointers (one 64-bit add per row instead of a 64-bit multiply-add chain)
     auto request_inputs = [&](long long cc) {
         if (cc < nc) {
             cp_async8(s_in, g.rho_g + cc);
+            const double* pd = g.rho_d + cc;
+            const double* pt = g.t_s + cc;
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
-                cp_async8(s_in + (1 + i) * kThreads, g.rho_d + i * nc + cc);
-                cp_async8(s_in + (1 + N + i) * kThreads, g.t_s + i * nc + cc);
+                cp_async8(s_in + (1 + i) * kThreads, pd);
+                cp_async8(s_in + (1 + N + i) * kThreads, pt);
+                pd += nc;
+                pt += nc;
             });
         }
         cp_async_commit();
@@ -67,9 +72,11 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
     while (cw < nc) {
         const bool valid = c < nc;
         if (valid) {
+            const double* pp = g.p_in + c;
             static_for<0, kRowsP>([&](auto R) {
                 constexpr int r = R;
-                cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
+                cp_async8(sp + r * kThreads, pp);
+                pp += nc;
             });
         }
         cp_async_commit();
@@ -125,8 +132,9 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
                         constexpr int k = K;
                         y = fma(P[Core::sx(i, k)], q[k], y);
                     });
-                    if constexpr (i == 0) po[0] = p[0] + y;
-                    else po[i * nc] = fma(w[i - 1], y, p[i]);
+                    if constexpr (i == 0) *po = p[0] + y;
+                    else *po = fma(w[i - 1], y, p[i]);
+                    po += nc;
                 });
             }
         }
@@ -154,22 +162,29 @@ __global__ void __launch_bounds__(kThreads, kRk1MinBlocks) k_rk1(UpdateArgs g) {
     const long long stride = (long long)gridDim.x * kThreads;
     long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
 
+    // row addresses by running pointers (one 64-bit add per row instead of a 64-bit multiply-add chain)
     auto request_inputs = [&](long long cc) {
         if (cc < nc) {
             cp_async8(s_in, g.rho_g + cc);
+            const double* pd = g.rho_d + cc;
+            const double* pt = g.t_s + cc;
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
-                cp_async8(s_in + (1 + i) * kThreads, g.rho_d + i * nc + cc);
-                cp_async8(s_in + (1 + N + i) * kThreads, g.t_s + i * nc + cc);
+                cp_async8(s_in + (1 + i) * kThreads, pd);
+                cp_async8(s_in + (1 + N + i) * kThreads, pt);
+                pd += nc;
+                pt += nc;
             });
         }
         cp_async_commit();
     };
     request_inputs(c);
     while (c < nc) {
+        const double* pp = g.p_in + c;
         static_for<0, kRowsP>([&](auto R) {
             constexpr int r = R;
-            cp_async8(sp + r * kThreads, g.p_in + r * nc + c);
+            cp_async8(sp + r * kThreads, pp);
+            pp += nc;
         });
         cp_async_commit();
         cp_async_wait<1>();  // the fields of cell c have landed
@@ -199,10 +214,11 @@ __global__ void __launch_bounds__(kThreads, kRk1MinBlocks) k_rk1(UpdateArgs g) {
             double B = b[0];
             static_for<0, N>([&](auto I) { B = fma(ci[I], b[I + 1], B); });
             const double q0 = B * iA;
-            po[0] = q0;
+            *po = q0;
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
-                po[(i + 1) * nc] = fma(ei[i], q0, gi[i] * b[i + 1]);
+                po += nc;
+                *po = fma(ei[i], q0, gi[i] * b[i + 1]);
             });
         }
         c = cn;
