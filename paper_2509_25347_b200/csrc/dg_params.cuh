@@ -113,9 +113,13 @@ __device__ __forceinline__ double fast_rsqrt(double x) {
     return fma(0.5 * y, e, y);
 }
 
+// max(x, lo) that lets a NaN through (fmax would return lo): the clamps of rounding noise must not hide a non-finite
+// input (include/dg.h: non-finite input gives non-finite output in that cell)
+__device__ __forceinline__ double clamp_below(double x, double lo) { return (x < lo) ? lo : x; }
+
 // 1/sqrt(eps) and sqrt(eps) with eps clamped away from zero so that rho_d = 0 stays finite (R12).
 __device__ __forceinline__ void sym_weights(double eps, double& w, double& iw) {
-    eps = fmax(eps, 1e-200);
+    eps = clamp_below(eps, 1e-200);
     iw = fast_rsqrt(eps);
     w = eps * iw;
 }

@@ -157,7 +157,7 @@ struct Tpc {
             constexpr int i = I;
             static_for<i + 1, n>([&](auto K) {
                 constexpr int k = K;
-                P[ix(i, k)] = fmax(P[ix(i, k)], 0.0);
+                P[ix(i, k)] = clamp_below(P[ix(i, k)], 0.0);
             });
         });
         conserve(P, w, iw);

@@ -292,8 +292,8 @@ struct Wpc {
 #pragma unroll
                 for (int J = 0; J < TL; ++J)
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) T[I][J][e] = fmax(T[I][J][e] * (bs * beC.v[J][e]), 0.0);
-                rR.v[I] = fmax(bs * vR.v[I], 0.0);
+                    for (int e = 0; e < 2; ++e) T[I][J][e] = clamp_below(T[I][J][e] * (bs * beC.v[J][e]), 0.0);
+                rR.v[I] = clamp_below(bs * vR.v[I], 0.0);
             }
         }
         row_to_col(L, rR, rC);

@@ -280,6 +280,34 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
                 assert abs(mpf(float(out[comp, k, c])) - ref[k]) <= PARITY_TOL * scale, (N, c, comp, k)
 
 
+@pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
+@pytest.mark.parametrize("variant", [0, 1, 2])
+def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
+    """include/dg.h: non-finite input gives non-finite output in that cell only.  With the thread-per-cell mapping
+    the poisoned cell shares a warp (and the warp's Taylor degree, R8) with 31 healthy ones: they must still
+    match the oracle."""
+    wl = W.make_workload(5, ncells=300, N=N, device=cuda)
+    bad = [7, 40, 41, 150, 299]
+    wl.t_s[0, 7] = float("nan")
+    wl.rho_g[40] = float("inf")
+    wl.p_in[1, N, 41] = float("nan")
+    wl.t_s[N - 1, 150] = 0.0            # a = dt / 0: infinite coupling rate
+    wl.rho_d[0, 299] = float("inf")
+    out = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=variant)[0]
+    torch.cuda.synchronize()
+    good = torch.ones(wl.ncells, dtype=torch.bool)
+    good[bad] = False
+    idx = torch.nonzero(good).flatten()
+    rho_g, rho_d, t_s, p_in = wl.cells(idx)
+    ref = oracle.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+    got = out[:, :, idx.to(cuda)].cpu().numpy()
+    assert np.isfinite(got).all()
+    assert float(oracle.parity_error(got, ref, p_in).max()) <= PARITY_TOL
+    for c in (7, 40, 150, 299):
+        assert not bool(torch.isfinite(out[:, :, c]).all()), c
+    assert not bool(torch.isfinite(out[1, :, 41]).all()) and bool(torch.isfinite(out[0, :, 41]).all())
+
+
 def test_equal_velocity_state_is_a_fixed_point(dg, cuda):
     """Omega rho = 0 (Eq. 17): momenta proportional to the densities do not change (long-time limit)."""
     for N in (1, 4, 8, 16):
