@@ -308,6 +308,29 @@ def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
     assert not bool(torch.isfinite(out[1, :, 41]).all()) and bool(torch.isfinite(out[0, :, 41]).all())
 
 
+@pytest.mark.parametrize("N,ncells", [(1, 33), (4, 127), (8, 1001), (13, 130), (16, 1027), (16, 3)])
+def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
+    """compute-sanitizer is not available on the GPU pool, so out-of-bounds writes are caught with canaries: p_out is
+    a window of a larger allocation whose borders must come back untouched, for every kernel that writes momenta."""
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
+    n = N + 1
+    guard = 4096
+    size = 3 * n * ncells
+    for which in ("tpc", "wpc", "paper", "rk1", "steps"):
+        big = torch.full((size + 2 * guard,), -7.25, dtype=torch.float64, device=cuda)
+        p_out = big[guard:guard + size].view(3, n, ncells)
+        if which == "rk1":
+            dg.dg_drag_rk1(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+        elif which == "steps":
+            dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 3, p_out=p_out)
+        else:
+            variant = {"tpc": 1, "wpc": 2, "paper": 3}[which]
+            dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=variant)
+        torch.cuda.synchronize()
+        assert bool((big[:guard] == -7.25).all()) and bool((big[guard + size:] == -7.25).all()), which
+        assert bool(torch.isfinite(p_out).all()) and not bool((p_out == -7.25).any()), which
+
+
 def test_equal_velocity_state_is_a_fixed_point(dg, cuda):
     """Omega rho = 0 (Eq. 17): momenta proportional to the densities do not change (long-time limit)."""
     for N in (1, 4, 8, 16):
