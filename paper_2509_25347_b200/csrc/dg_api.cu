@@ -26,10 +26,11 @@ static const PaperLaunchers* const kPaperTable[DG_NMAX + 1] = {
     &paper_launchers_N10, &paper_launchers_N11, &paper_launchers_N12, &paper_launchers_N13, &paper_launchers_N14,
     &paper_launchers_N15, &paper_launchers_N16};
 
-// The mapping dg_drag_update uses for each N, chosen from measurements on B200: registers hold the
-// packed symmetric matrices of one cell per thread up to N = 12; beyond that the thread-per-cell kernel spills and the
-// warp-per-cell DMMA kernel wins.
-constexpr int kFirstWpcN = 13;
+// The mapping dg_drag_update uses for each N, chosen from measurements on B200: the thread-per-cell
+// kernel keeps the packed symmetric matrices of one cell in registers up to N = 9 and spills mildly up to N = 13, where
+// it still wins (2^21 stiff cells: 8.1 vs 11.3 ms at N = 13, 21.5 vs 11.4 ms at N = 14); from N = 14 its spills take
+// over and the warp-per-cell DMMA kernel wins.
+constexpr int kFirstWpcN = 14;
 static inline int default_variant(int N) { return N >= kFirstWpcN ? DG_VARIANT_WPC : DG_VARIANT_TPC; }
 
 static thread_local char g_cuda_err[256] = "";
