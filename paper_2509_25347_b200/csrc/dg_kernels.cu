@@ -105,35 +105,44 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
         // a2-a4
         double P[SZ];
         int m, s;
-        Core::expm(a, w, iw, P, m, s);
+        Core::template expm<Core::kDeferLast>(a, w, iw, P, m, s);
         if (valid) {
             if (g.s_out) g.s_out[c] = s;
             if (g.m_out) g.m_out[c] = m;
         }
 
-        // a5: p_out = p_in + W P W^-1 p_in, one component at a time
+        // a5: p_out = p_in + W P W^-1 p_in, one component at a time; applied twice where the last squaring was
+        // deferred (dg_tpc.cuh)
         cp_async_wait<1>();  // the momenta of cell c have landed (the next cell's inputs may still be in flight)
         if (valid) {
+            const bool twice = Core::kDeferLast && s > 0;
 #pragma unroll 1
             for (int comp = 0; comp < 3; ++comp) {
                 const double* pi = sp + comp * n * kThreads;
                 double* po = g.p_out + (long long)comp * n * nc + c;
                 double p[n], q[n];
-                static_for<0, n>([&](auto K) {
-                    constexpr int k = K;
-                    p[k] = pi[k * kThreads];
-                    if constexpr (k == 0) q[k] = p[k];
-                    else q[k] = p[k] * iw[k - 1];
-                });
-                static_for<0, n>([&](auto I) {
-                    constexpr int i = I;
-                    double y = 0.0;
+                static_for<0, n>([&](auto K) { p[K] = pi[K * kThreads]; });
+                auto apply_once = [&]() {
                     static_for<0, n>([&](auto K) {
                         constexpr int k = K;
-                        y = fma(P[Core::sx(i, k)], q[k], y);
+                        if constexpr (k == 0) q[k] = p[k];
+                        else q[k] = p[k] * iw[k - 1];
                     });
-                    if constexpr (i == 0) *po = p[0] + y;
-                    else *po = fma(w[i - 1], y, p[i]);
+                    static_for<0, n>([&](auto I) {
+                        constexpr int i = I;
+                        double y = 0.0;
+                        static_for<0, n>([&](auto K) {
+                            constexpr int k = K;
+                            y = fma(P[Core::sx(i, k)], q[k], y);
+                        });
+                        if constexpr (i == 0) p[0] = p[0] + y;
+                        else p[i] = fma(w[i - 1], y, p[i]);
+                    });
+                };
+                apply_once();
+                if (twice) apply_once();
+                static_for<0, n>([&](auto I) {
+                    *po = p[I];
                     po += nc;
                 });
             }

@@ -71,6 +71,16 @@ struct Tpc {
 
     // a[i] = dt/t_s,i (unscaled), w[i] = sqrt(eps_i), iw[i] = 1/w[i].  On return P holds exp(S) - I (packed, diagonal
     // slots = d) and m, s are the chosen Taylor degree and scaling exponent.
+    // The fused kernel does not need exp(S) itself, only exp(S) applied to three vectors: for n > 6 a squaring
+    // (~n^3/2 fp64 instructions) costs more than a second apply (3 n^2), so with kDeferLast the LAST squaring is left
+    // out here and the caller applies X_{s-1} twice,  exp(S) q = X_{s-1} (X_{s-1} q).  X_{s-1} has had its diagonal
+    // re-derived from conservation, so each of the two applies conserves total momentum to rounding.
+    static constexpr bool kDeferLast = (N >= 6);
+
+    // a[i] = dt/t_s,i (unscaled), w[i] = sqrt(eps_i), iw[i] = 1/w[i].  On return m, s are the chosen Taylor degree and
+    // scaling exponent and P holds X - I (packed, diagonal slots = d) with X = exp(S) — or, if defer_last and s > 0,
+    // X = exp(S/2), the iterate before the last squaring.
+    template <bool defer_last = false>
     __device__ __forceinline__ static void expm(const double (&a)[N], const double (&w)[N], const double (&iw)[N],
                                                 double (&P)[SZ], int& m, int& s) {
         // The scaling exponent is chosen on ||S||_2 (Theorem 1, holds in any consistent norm; S is
@@ -163,7 +173,7 @@ struct Tpc {
         conserve(P, w, iw);
 
         // s squarings: O <- offdiag(X X), X = O + diag(1 + d) >= 0 entrywise, X symmetric
-        for (int it = 0; it < s; ++it) {
+        for (int it = defer_last ? 1 : 0; it < s; ++it) {
             double X[SZ];
             static_for<0, SZ>([&](auto K) { X[K] = P[K]; });
             static_for<0, n>([&](auto I) {
