@@ -78,10 +78,11 @@ def useful_flops(N, s, m):
     apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)
     sm = s.double()
     mm = m.double()
-    # thread-per-cell kernels with n > 6 leave the last squaring out and apply X_{s-1} twice (dg_tpc.cuh kDeferLast)
-    deferred = ((sm > 0) & (6 <= N <= 13)).double() if 6 <= N <= 13 else torch.zeros_like(sm)
+    # thread-per-cell kernels with 6 <= N <= 10 leave the last squaring out and apply X_{s-1} twice (dg_tpc.cuh kDefer)
+    kdef = 1 if 6 <= N <= 10 else 0
+    deferred = sm.clamp(max=kdef)
     per_cell = (build + first + (mm - 1).clamp(min=0) * horner + tri + conserve + (sm - deferred) * square
-                + (1.0 + deferred) * apply_)
+                + torch.pow(2.0, deferred) * apply_)
     return float(per_cell.sum().item())
 
 

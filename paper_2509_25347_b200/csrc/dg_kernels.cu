@@ -105,17 +105,17 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
         // a2-a4
         double P[SZ];
         int m, s;
-        Core::template expm<Core::kDeferLast>(a, w, iw, P, m, s);
+        Core::template expm<Core::kDefer>(a, w, iw, P, m, s);
         if (valid) {
             if (g.s_out) g.s_out[c] = s;
             if (g.m_out) g.m_out[c] = m;
         }
 
-        // a5: p_out = p_in + W P W^-1 p_in, one component at a time; applied twice where the last squaring was
-        // deferred (dg_tpc.cuh)
+        // a5: p_out = p_in + W P W^-1 p_in, one component at a time; applied 2^k times where the last k squarings were
+        // left out (dg_tpc.cuh kDefer)
         cp_async_wait<1>();  // the momenta of cell c have landed (the next cell's inputs may still be in flight)
         if (valid) {
-            const bool twice = Core::kDeferLast && s > 0;
+            const int napply = 1 << min(Core::kDefer, s);
 #pragma unroll 1
             for (int comp = 0; comp < 3; ++comp) {
                 const double* pi = sp + comp * n * kThreads;
@@ -139,8 +139,8 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
                         else p[i] = fma(w[i - 1], y, p[i]);
                     });
                 };
-                apply_once();
-                if (twice) apply_once();
+#pragma unroll 1
+                for (int rep = 0; rep < napply; ++rep) apply_once();
                 static_for<0, n>([&](auto I) {
                     *po = p[I];
                     po += nc;

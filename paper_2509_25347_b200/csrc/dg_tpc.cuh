@@ -71,16 +71,17 @@ struct Tpc {
 
     // a[i] = dt/t_s,i (unscaled), w[i] = sqrt(eps_i), iw[i] = 1/w[i].  On return P holds exp(S) - I (packed, diagonal
     // slots = d) and m, s are the chosen Taylor degree and scaling exponent.
-    // The fused kernel does not need exp(S) itself, only exp(S) applied to three vectors: for n > 6 a squaring
-    // (~n^3/2 fp64 instructions) costs more than a second apply (3 n^2), so with kDeferLast the LAST squaring is left
-    // out here and the caller applies X_{s-1} twice,  exp(S) q = X_{s-1} (X_{s-1} q).  X_{s-1} has had its diagonal
-    // re-derived from conservation, so each of the two applies conserves total momentum to rounding.
-    static constexpr bool kDeferLast = (N >= 6);
+    // The fused kernel does not need exp(S) itself, only exp(S) applied to three vectors.  A squaring costs ~n^3/2
+    // fp64 instructions, an apply 3 n^2: for n > 6 it is cheaper to leave the LAST squaring out and apply X_{s-1}
+    // twice, exp(S) q = X_{s-1} (X_{s-1} q).  Measured: 2-4 % faster for N = 6..10; from N = 11, where P spills, the
+    // second apply costs what it saves (and leaving two squarings out for four applies is 5 % slower), so not there.
+    // Every X_k has had its diagonal re-derived from conservation, so each apply conserves total momentum to rounding.
+    static constexpr int kDefer = (N >= 6 && N <= 10) ? 1 : 0;
 
     // a[i] = dt/t_s,i (unscaled), w[i] = sqrt(eps_i), iw[i] = 1/w[i].  On return m, s are the chosen Taylor degree and
-    // scaling exponent and P holds X - I (packed, diagonal slots = d) with X = exp(S) — or, if defer_last and s > 0,
-    // X = exp(S/2), the iterate before the last squaring.
-    template <bool defer_last = false>
+    // scaling exponent and P holds X - I (packed, diagonal slots = d) with X = exp(S / 2^min(defer, s)): exp(S) itself
+    // for defer = 0, the iterate min(defer, s) squarings short of it otherwise.
+    template <int defer = 0>
     __device__ __forceinline__ static void expm(const double (&a)[N], const double (&w)[N], const double (&iw)[N],
                                                 double (&P)[SZ], int& m, int& s) {
         // The scaling exponent is chosen on ||S||_2 (Theorem 1, holds in any consistent norm; S is
@@ -173,7 +174,7 @@ struct Tpc {
         conserve(P, w, iw);
 
         // s squarings: O <- offdiag(X X), X = O + diag(1 + d) >= 0 entrywise, X symmetric
-        for (int it = defer_last ? 1 : 0; it < s; ++it) {
+        for (int it = min(defer, s); it < s; ++it) {
             double X[SZ];
             static_for<0, SZ>([&](auto K) { X[K] = P[K]; });
             static_for<0, n>([&](auto I) {
