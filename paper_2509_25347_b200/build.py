@@ -5,8 +5,8 @@
 One object per translation unit, compiled in parallel: dg_kernels.cu, dg_wpc_kernels.cu and dg_paper_kernels.cu once
 per species count N (-DDG_N=<N>), plus
 dg_api.cu, dg_peaks.cu, dg_host.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
-nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 division, sqrt and the exponent arithmetic must stay
-IEEE.
+nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 arithmetic must stay IEEE (the kernels' own Newton
+reciprocals are explicit, dg_params.cuh).  Extra nvcc flags for an experiment can be passed in DG_EXTRA_FLAGS.
 """
 import argparse
 import os
