@@ -127,7 +127,10 @@ def test_full_size_sampled(dg, oracle, cuda, config):
     """BASELINE.json's full cell counts (128^3 / 256^3): parity on a strided sample of cells the oracle computes one
     by one, conservation on EVERY cell (needs no oracle; fp64 sums on the device, rounding ~n*u << 1e-13)."""
     wl = W.make_workload(config, device=cuda)
-    idx = W.sample_cells(wl.ncells, 2048)
+    # a strided sample plus the 256 stiffest cells of the whole array (largest ||A||_1: the most squarings)
+    norm1 = 2.0 * torch.maximum((wl.rho_d / wl.rho_g[None, :] * (wl.dt / wl.t_s)).sum(dim=0), (wl.dt / wl.t_s).amax(dim=0))
+    stiffest = torch.topk(norm1, 256).indices.cpu()
+    idx = torch.unique(torch.cat([W.sample_cells(wl.ncells, 2048), stiffest]))
     run_and_compare(dg, oracle, wl, idx=idx)
     out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
     drift = (out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)
