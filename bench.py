@@ -73,7 +73,7 @@ def useful_flops(N, s, m):
               + N * (N - 1)                      # U_ik <- v_k - alpha_i U_ik: one fma per packed dust entry
               + (2 * N - 1)                      # sum_l beta_l^2 v_l: one mul + (N-1) fma
               + 1 + 2 * N + 2)                   # kappa_j + Q_00; v_k <- x00 - alpha_k v_k (fma each); Q_00 (fma)
-    conserve = (2 * N + 1) + N * (1 + 2 * (N - 1) + 1)
+    conserve = (2 * N - 1) * n                   # per column: (N-1) fma and one mul
     square = n + tri * (1 + 2 * N) + conserve    # 1 + d; offdiag(X X): mul + N fma per entry; diagonal from conservation
     apply_ = 3 * (N + 2 * n * n + 1 + 2 * N)
     sm = s.double()

@@ -56,21 +56,24 @@ struct Tpc {
     __device__ __forceinline__ static void conserve(double (&P)[SZ], const double (&w)[N], const double (&iw)[N]) {
         static_for<0, n>([&](auto J) {
             constexpr int j = J;
-            double acc = 0.0;
-            static_for<0, n>([&](auto I) {
-                constexpr int i = I;
-                if constexpr (i != j) {
-                    if constexpr (i == 0) acc += P[sx(0, j)];
-                    else acc = fma(w[i - 1], P[sx(i, j)], acc);
-                }
-            });
-            if constexpr (j == 0) P[ix(0, 0)] = -acc;
-            else P[ix(j, j)] = -acc * iw[j - 1];
+            if constexpr (j == 0) {
+                double acc = w[0] * P[ix(0, 1)];
+                static_for<2, n>([&](auto I) {
+                    constexpr int i = I;
+                    acc = fma(w[i - 1], P[ix(0, i)], acc);
+                });
+                P[ix(0, 0)] = -acc;
+            } else {
+                double acc = P[ix(0, j)];  // w_0 = 1
+                static_for<1, n>([&](auto I) {
+                    constexpr int i = I;
+                    if constexpr (i != j) acc = fma(w[i - 1], P[sx(i, j)], acc);
+                });
+                P[ix(j, j)] = -acc * iw[j - 1];
+            }
         });
     }
 
-    // a[i] = dt/t_s,i (unscaled), w[i] = sqrt(eps_i), iw[i] = 1/w[i].  On return P holds exp(S) - I (packed, diagonal
-    // slots = d) and m, s are the chosen Taylor degree and scaling exponent.
     // The fused kernel does not need exp(S) itself, only exp(S) applied to three vectors.  A squaring costs ~n^3/2
     // fp64 instructions, an apply 3 n^2: for n > 6 it is cheaper to leave the LAST squaring out and apply X_{s-1}
     // twice, exp(S) q = X_{s-1} (X_{s-1} q).  Measured: 2-4 % faster for N = 6..10; from N = 11, where P spills, the
