@@ -334,6 +334,33 @@ def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
         assert bool(torch.isfinite(p_out).all()) and not bool((p_out == -7.25).any()), which
 
 
+@pytest.mark.parametrize("N", [2, 8, 16])
+def test_cuda_graph_capture_and_second_stream(dg, cuda, N):
+    """The entry points only enqueue work on the caller's stream (include/dg.h): a multi-step drag sequence can be
+    captured into a CUDA graph and replayed, and a launch on a side stream gives the same bits as on the default one."""
+    wl = W.make_workload(5, ncells=5000 + N, N=N, device=cuda)
+    ref = dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 4)   # also warms the one-time set-up
+    ref_rk1 = dg.dg_drag_rk1(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    torch.cuda.synchronize()
+    out = torch.empty_like(wl.p_in)
+    out_rk1 = torch.empty_like(wl.p_in)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 4, p_out=out)
+        dg.dg_drag_rk1(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=out_rk1)
+    for _ in range(2):
+        out.zero_(); out_rk1.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref) and torch.equal(out_rk1, ref_rk1)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        out2 = dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 4)
+    side.synchronize()
+    assert torch.equal(out2, ref)
+
+
 def test_equal_velocity_state_is_a_fixed_point(dg, cuda):
     """Omega rho = 0 (Eq. 17): momenta proportional to the densities do not change (long-time limit)."""
     for N in (1, 4, 8, 16):
