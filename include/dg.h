@@ -27,12 +27,20 @@
  *
  * Streams and asynchrony.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  * entry points only enqueue work and return; they never synchronise.  They are re-entrant and may be called
- * concurrently on different streams.  Results are bitwise reproducible for a fixed build and GPU.
+ * concurrently on different streams.
+ *
+ * Reproducibility.  For a fixed build and GPU the same call (same pointers' cell ranges, same ncells) gives the same
+ * bits, run to run.  A cell's VALUE never depends on other cells beyond rounding: every cell agrees with the exact
+ * result to the documented tolerance whatever its neighbours hold.  Its BITS may: the kernels pick the Taylor degree m
+ * (any Table B.1 row is admissible for any cell) once per group of cells that share a warp, so computing the same
+ * cell as part of a different sub-range of the arrays (another offset or ncells) may change its result at O(u).
+ * dg_drag_update_host cuts its chunks so that it stays bit-identical to one dg_drag_update over all cells.
  *
  * Errors.  Every entry point returns a dg_status; nothing throws or aborts across the ABI:
  *     DG_ENULL   a required pointer is NULL (checked only when ncells > 0)
  *     DG_ERANGE  N outside [1, DG_NMAX] or ncells < 0
- *     DG_EALIGN  a pointer is not 8-byte aligned
+ *     DG_EALIGN  a pointer is not 8-byte aligned (fp64 arrays; 4-byte for the int32 arrays).  8 bytes is all that is
+ *                required; 16-byte aligned base pointers with an even ncells let some kernels move two cells per copy
  *     DG_EINVAL  dt negative or not finite, or another scalar argument outside its documented range
  *     DG_ECUDA   the CUDA runtime reported an error (cudaGetLastError after the launch, or a failed copy/alloc);
  *                dg_last_cuda_error() returns its text

@@ -125,7 +125,12 @@ __global__ void __launch_bounds__(kThreads, 3) k_update_wpc(UpdateArgs g) {
     const long long nc = g.ncells;
     const long long ngroups = (nc + kGroup - 1) / kGroup;
     const long long gstride = (long long)gridDim.x * kWarps;
-    const bool vec16 = (nc & 1) == 0;
+    // 16-byte copies need every row start 16-byte aligned: an even cell count AND 16-byte aligned base pointers (the ABI
+    // only asks for 8: include/dg.h); otherwise the element-by-element path
+    const bool vec16 = (nc & 1) == 0 &&
+                       ((reinterpret_cast<unsigned long long>(g.rho_g) | reinterpret_cast<unsigned long long>(g.rho_d) |
+                         reinterpret_cast<unsigned long long>(g.t_s) | reinterpret_cast<unsigned long long>(g.p_in) |
+                         reinterpret_cast<unsigned long long>(g.p_out)) & 15ull) == 0;
     long long grp = (long long)blockIdx.x * kWarps + warp;
     int stage = 0;
     request_group(g, sm.in[0], grp * kGroup, lane, vec16);
@@ -305,34 +310,45 @@ __global__ void __launch_bounds__(kThreads) k_expm_wpc(ExpmArgs g) {
     }
 }
 
-unsigned persistent_grid(const void* kernel, long long units, size_t smem) {
-    int dev = 0, sms = 148, per_sm = 1;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, smem);
-    if (per_sm < 1) per_sm = 1;
-    long long want = (units + kWarps - 1) / kWarps;
-    long long cap = (long long)sms * per_sm;
-    return (unsigned)(want < cap ? want : cap);
-}
-
-cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    static bool configured[64] = {false};  // per device
+// Persistent grid: as many blocks as fit on the device at once (or fewer, if there is not enough work).  The
+// occupancy query and the shared-memory opt-in are done once per device and cached (`cap` = blocks per device).
+cudaError_t persistent_grid(const void* kernel, size_t smem, long long (&cap)[64], long long units, unsigned* grid) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (!configured[dev]) {
-        e = cudaFuncSetAttribute(k_update_wpc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (cap[dev] == 0) {
+        int sms = 0, per_sm = 0;
+        if (smem > 0) {
+            e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
-        configured[dev] = true;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, smem);
+        if (e != cudaSuccess) return e;
+        cap[dev] = (long long)sms * (per_sm > 0 ? per_sm : 1);
     }
+    const long long want = (units + kWarps - 1) / kWarps;
+    *grid = (unsigned)(want < cap[dev] ? want : cap[dev]);
+    return cudaSuccess;
+}
+
+cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
+    static long long cap[64] = {0};  // per device; 0 = not yet queried
+    unsigned grid = 0;
     const long long ngroups = (a.ncells + kGroup - 1) / kGroup;
-    k_update_wpc<<<persistent_grid((const void*)k_update_wpc, ngroups, kSmemBytes), kThreads, kSmemBytes, st>>>(a);
+    cudaError_t e = persistent_grid((const void*)k_update_wpc, kSmemBytes, cap, ngroups, &grid);
+    if (e != cudaSuccess) return e;
+    k_update_wpc<<<grid, kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError();
 }
 cudaError_t launch_expm(const ExpmArgs& a, cudaStream_t st) {
-    k_expm_wpc<<<persistent_grid((const void*)k_expm_wpc, a.ncells, 0), kThreads, 0, st>>>(a);
+    static long long cap[64] = {0};
+    unsigned grid = 0;
+    cudaError_t e = persistent_grid((const void*)k_expm_wpc, 0, cap, a.ncells, &grid);
+    if (e != cudaSuccess) return e;
+    k_expm_wpc<<<grid, kThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -258,18 +258,23 @@ def test_extreme_stiffness_and_weak_coupling(dg, oracle, cuda, N):
     assert (np.abs(got).max(axis=1) <= np.abs(p_in).sum(axis=1) * (1 + 1e-12)).all()
 
 
-@pytest.mark.parametrize("N", [1, 2, 5])
+@pytest.mark.parametrize("N", [1, 2, 5, 8, 16])
 def test_extreme_stiffness_against_mpmath(dg, cuda, N):
     """The stiffest cells (dt/t_s = 1e10, ~40 squarings) against mpmath.expm at 90 digits applied to Eq. 17
-     retyped here: an arbitrary-precision reference that is neither the oracle nor the CUDA path."""
+     retyped here: an arbitrary-precision reference that is neither the oracle nor the CUDA path.
+    N = 8 and 16 run every thread mapping: the default one, thread-per-cell (for N = 8 with the last squaring replaced
+    by a second apply) and the warp-per-cell DMMA kernel, whose diagonal is re-derived from conservation on every other
+    squaring only (Eq. 23-24; Theorem 1)."""
     import mpmath as mpm
     from mpmath import mp, mpf
     mp.dps = 90
     wl = _extreme_workload(N, cuda)
-    out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in).cpu().numpy()
+    variants = (0,) if N < 8 else (0, 1, 2)
+    outs = {v: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=v) for v in variants}
     rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(wl.ncells))
     n = N + 1
-    for c in (64, 77, 101, 127, 300):
+    cells = (64, 77, 101, 127, 300) if N < 8 else (64, 101, 127, 300)
+    for c in cells:
         A = mpm.zeros(n, n)
         for i in range(N):
             alpha = mpf(wl.dt) / mpf(float(t_s[i, c]))
@@ -277,10 +282,47 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
             A[0, 0] -= e * alpha; A[0, i + 1] = alpha; A[i + 1, 0] = e * alpha; A[i + 1, i + 1] = -alpha
         E = mpm.expm(A, method="taylor")
         scale = max(abs(float(x)) for x in p_in[:, :, c].ravel())
-        for comp in range(3):
-            ref = E * mpm.matrix([mpf(float(x)) for x in p_in[comp, :, c]])
-            for k in range(n):
-                assert abs(mpf(float(out[comp, k, c])) - ref[k]) <= PARITY_TOL * scale, (N, c, comp, k)
+        refs = [E * mpm.matrix([mpf(float(x)) for x in p_in[comp, :, c]]) for comp in range(3)]
+        for v, (out, s, m) in outs.items():
+            if c < 128:
+                assert int(s[c]) >= 30, (N, c, v, int(s[c]))      # these are the ~1e10-norm cells
+            o = out[:, :, c].cpu().numpy()
+            for comp in range(3):
+                for k in range(n):
+                    assert abs(mpf(float(o[comp, k])) - refs[comp][k]) <= PARITY_TOL * scale, (N, c, v, comp, k)
+
+
+@pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0)])
+@pytest.mark.parametrize("ncells", [512, 515, 2050])
+def test_pointers_that_are_8_but_not_16_byte_aligned(dg, oracle, cuda, N, variant, ncells):
+    """include/dg.h asks for 8-byte alignment only.  Every array is a view starting one double into its allocation
+    (8 mod 16), with even and odd cell counts: the kernels that move two cells per 16-byte copy must fall back to
+    8-byte accesses instead of faulting, and the results must still match the oracle."""
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
+
+    def shifted(t):
+        big = torch.empty(t.numel() + 3, dtype=t.dtype, device=t.device)
+        v = big[1:1 + t.numel()].view(t.shape)
+        v.copy_(t)
+        assert v.data_ptr() % 16 == 8 and v.is_contiguous()
+        return v
+
+    rho_g, rho_d, t_s, p_in = (shifted(t) for t in (wl.rho_g, wl.rho_d, wl.t_s, wl.p_in))
+    p_out = shifted(torch.zeros_like(wl.p_in))
+    dg.dg_drag_update_ex(rho_g, rho_d, t_s, wl.dt, p_in, p_out=p_out, variant=variant)
+    torch.cuda.synchronize()
+    ref_dev = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=variant)[0]
+    assert torch.equal(p_out, ref_dev)                    # same bits as the 16-byte aligned call
+    h = wl.cells(torch.arange(wl.ncells))
+    ref = oracle.drag_update(h[0], h[1], h[2], wl.dt, h[3])
+    assert float(oracle.parity_error(p_out.cpu().numpy(), ref, h[3]).max()) <= PARITY_TOL
+    # one array at a time misaligned (the others 16-byte aligned)
+    for which in range(5):
+        args = [wl.rho_g, wl.rho_d, wl.t_s, wl.p_in, torch.zeros_like(wl.p_in)]
+        args[which] = shifted(args[which])
+        dg.dg_drag_update_ex(args[0], args[1], args[2], wl.dt, args[3], p_out=args[4], variant=variant)
+        torch.cuda.synchronize()
+        assert torch.equal(args[4], ref_dev), which
 
 
 @pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
