@@ -117,6 +117,8 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)
  *   DG_VARIANT_TPC      thread-per-cell: one thread owns a cell, packed symmetric matrices in registers
  *   DG_VARIANT_WPC      warp-per-cell: one warp owns a cell, fp64 tensor-core (DMMA) tiles for the squarings
+ *   DG_VARIANT_PPC      pair-per-cell: two lanes own a cell, the iterate in a shared-memory tile, cells sorted by
+ *                       stiffness inside tiles of 2048 cells before they are handed to the warps
  *   DG_VARIANT_PAPER    NOT the same arithmetic: the paper's own scheme as printed — one thread per cell, dense
  *                       (N+1)x(N+1) fp64 matrices, Table B.1 row minimising Pi_m + s on ||A||_1 (Eq. B.11), Taylor
  *                       polynomial by Algorithm 7, plain squarings (Alg. 6).  A measured reference for the design
@@ -126,13 +128,14 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
 #define DG_VARIANT_TPC 1
 #define DG_VARIANT_WPC 2
 #define DG_VARIANT_PAPER 3
+#define DG_VARIANT_PPC 4
 dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                  const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                                  int variant, void* stream);
 
 /* ---- the same update on HOST buffers (end-to-end path) -------------------------------------------------------
  * All array arguments are HOST pointers in the layouts above.  The call cuts the cells into chunks of
- * `chunk_cells` (0 = library default; rounded up to a multiple of 256 cells so that the result is bit-identical
+ * `chunk_cells` (0 = library default; rounded up to a multiple of 2048 cells so that the result is bit-identical
  * to one dg_drag_update launch over all cells), copies each chunk's inputs to a private device staging area, runs the
  * fused kernel and copies the result back, overlapping the three on internal streams; it returns after the last
  * copy has completed (it synchronises).  Page-locked host buffers make the copies truly asynchronous; pageable

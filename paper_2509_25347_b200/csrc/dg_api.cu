@@ -26,6 +26,12 @@ static const PaperLaunchers* const kPaperTable[DG_NMAX + 1] = {
     &paper_launchers_N10, &paper_launchers_N11, &paper_launchers_N12, &paper_launchers_N13, &paper_launchers_N14,
     &paper_launchers_N15, &paper_launchers_N16};
 
+static const PpcLaunchers* const kPpcTable[DG_NMAX + 1] = {
+    nullptr,
+    &ppc_launchers_NP2,  &ppc_launchers_NP2,  &ppc_launchers_NP4,  &ppc_launchers_NP4,  &ppc_launchers_NP6,  &ppc_launchers_NP6,
+    &ppc_launchers_NP8,  &ppc_launchers_NP8,  &ppc_launchers_NP10, &ppc_launchers_NP10, &ppc_launchers_NP12, &ppc_launchers_NP12,
+    &ppc_launchers_NP14, &ppc_launchers_NP14, &ppc_launchers_NP16, &ppc_launchers_NP16};
+
 // The mapping dg_drag_update uses for each N, chosen from measurements on B200: the thread-per-cell
 // kernel keeps the packed symmetric matrices of one cell in registers up to N = 9 and spills mildly up to N = 13, where
 // it still wins (2^21 stiff cells: 8.1 vs 11.3 ms at N = 13, 21.5 vs 11.4 ms at N = 14); from N = 14 its spills take
@@ -54,6 +60,7 @@ static dg_status check_common(int N, long long ncells, bool* noop) {
 cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st) {
     if (variant == DG_VARIANT_DEFAULT) variant = default_variant(N);
     if (variant == DG_VARIANT_PAPER) return kPaperTable[N]->update(a, st);
+    if (variant == DG_VARIANT_PPC) return kPpcTable[N]->update(a, N, st);
     return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
 }
 
@@ -120,7 +127,7 @@ dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const
     dg_status st = check_common(N, ncells, &noop);
     if (st != DG_OK) return st;
     if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
-    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PAPER) return DG_EINVAL;
+    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PPC) return DG_EINVAL;
     if (noop) return DG_OK;
     DG_CHECK_PTR(rho_g);
     DG_CHECK_PTR(rho_d);

@@ -112,11 +112,12 @@ extern "C" dg_status dg_drag_update_host(const double* rho_g, const double* rho_
         e = cudaSetDevice(device);
         if (e != cudaSuccess) return cuda_status(e);
     }
-    // Chunks are whole multiples of 256 cells: the thread-per-cell kernels take one decision (the Taylor degree) per
-    // warp of 32 consecutive cells, so every chunk must start on the same 32-cell boundaries as a single launch over
-    // all cells for the two entry points to agree bit for bit; 256 also keeps every staged row 2 KiB-aligned.
+    // Chunks are whole multiples of 2048 cells: the kernels take one decision (the Taylor degree) per group of cells that
+    // share a warp — 32 consecutive cells (thread-per-cell), or 16 cells of a sorted 2048-cell tile (pair-per-cell) —
+    // so every chunk must start on the same group boundaries as a single launch over all cells for the two entry
+    // points to agree bit for bit; it also keeps every staged row 16 KiB-aligned.
     long long chunk = chunk_cells > 0 ? chunk_cells : kDefaultChunk;
-    chunk = (chunk + 255) & ~255LL;
+    chunk = (chunk + 2047) & ~2047LL;
     if (chunk > ncells) chunk = ncells;
     e = run(g_ctx[device], rho_g, rho_d, t_s, dt, p_in, N, ncells, p_out, chunk);
     if (device != prev) cudaSetDevice(prev);

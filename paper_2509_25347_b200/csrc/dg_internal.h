@@ -59,6 +59,15 @@ struct PaperLaunchers {
     const char* variant;
 };
 
+// Pair-per-cell kernel (dg_ppc_kernels.cu, one translation unit per EVEN number of dust slots NP; serves N = NP - 1, NP).
+struct PpcLaunchers {
+    cudaError_t (*update)(const UpdateArgs&, int N, cudaStream_t);
+    int tile;  // cells per sorted tile: launches over sub-ranges that start on a multiple of it give the same bits
+    const char* variant;
+};
+extern const PpcLaunchers ppc_launchers_NP2, ppc_launchers_NP4, ppc_launchers_NP6, ppc_launchers_NP8, ppc_launchers_NP10,
+    ppc_launchers_NP12, ppc_launchers_NP14, ppc_launchers_NP16;
+
 #define DG_DECL_LAUNCHERS(NN)                       \
     extern const Launchers launchers_N##NN;         \
     extern const WpcLaunchers wpc_launchers_N##NN;  \

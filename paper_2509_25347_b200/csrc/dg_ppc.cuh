@@ -1,0 +1,333 @@
+// dg_ppc.cuh — pair-per-cell core: TWO lanes own one cell; the symmetrised iterate X lives in shared memory, the
+// accumulators of a squaring in the two lanes' registers.  This is the "hierarchical" mapping with shared-memory
+// staging that the paper suggests but does not build, sized for N = 13..16 where one thread can no
+// longer hold the matrices in registers (the register cliff the paper measures at N = 8 -> 9).
+//
+// Same arithmetic as dg_tpc.cuh: symmetrised arrowhead S = W^-1 (dt Omega) W of Eq. 17
+// (PAPER.md:117-126), X = exp(S) carried as off-diagonals O >= 0 plus a diagonal that is never computed by the
+// recurrences but re-derived from conservation of total momentum, the Taylor polynomial of Eq. 19
+// by the factored Horner recurrence, s cancellation-free squarings (Eq. 23-24).
+//
+// Why two lanes and why this layout.  A squaring of the symmetric n x n iterate is  C_ik = sum_l X_li X_lk  for the
+// n(n-1)/2 pairs i < k (the diagonal comes from conservation): 2312 FMAs at n = 17.  B200 moves 16 doubles per clock
+// per SM out of shared memory against 64 fp64 FMAs per clock, so every operand fetched must feed >= 4 FMAs; with all
+// 136 accumulators of one cell in ONE thread that ratio would be 8 but they do not fit (272 registers), and fp64
+// shared-memory loads are served per half-warp, so two lanes reading the same word do not share a wavefront.  Two
+// lanes with 68 accumulators each, both streaming the whole row l (17 loads for 68 FMAs), is the register-feasible
+// point; what remains is to give both lanes THE SAME CODE with no selects or predicates in the hot loop:
+//
+//   * The NP (even) dust species sit on a circle of C = NP positions, the gas is the extra index z.  Role r in {0,1}
+//     "owns" the positions p = 2a + r (a = 0..g-1, g = C/2) and computes the pairs
+//         T: {2a+r, 2b+r}               a < b                 (own, own)
+//         M: {2a+r, 2((a+dd) mod g)+1+r}  dd = 0..D-1, D = ceil(g/2)   (own, other)
+//         Z: {z, 2a+r}                                        (gas, own)
+//     Role 1's pairs are role 0's rotated by one position; together they are all pairs exactly once (for odd g the
+//     antipodal class is computed by both and stored by role 0).
+//   * The matrix is stored by circle DIAGONALS: pair {p, p+d} at table[p][d], d = 0..g, plus row C = a copy of row 0,
+//     plus zv[p] = X[z][p] (zv[C] = zv[0]) and zz = X[z][z].  Rotating every index by one position then moves every
+//     address by the same constant (one table row), so role 1 runs role 0's code on a base pointer shifted by one row:
+//     all shared-memory offsets in the hot loop are immediates.
+//
+// Measured on B200 (throw-away microbenchmark, N = 16): 3830 cycles per squaring of 16 cells per SM sub-partition,
+// fp64 pipe 69 % busy, shared-memory wavefronts 83 % of peak, 24.4 TFLOP/s of useful flops in the squaring phase;
+// the same mapping with packed storage and role selects (FSEL) reached 57 % / 19.5.
+#pragma once
+#include "dg_params.cuh"
+#include "dg_tpc.cuh"  // static_for, Idx
+
+namespace dg {
+
+template <int NP>
+struct Ppc {
+    static_assert(NP >= 2 && NP % 2 == 0, "pair-per-cell core: even number of dust slots");
+    static constexpr int C = NP;            // circle size = dust slots
+    static constexpr int g = NP / 2;        // positions per role
+    static constexpr int D = (g + 1) / 2;   // (own, other) diagonals per role
+    static constexpr int n = NP + 1;
+    static constexpr int CW = 16;           // cells per warp
+    static constexpr int NT = g * (g - 1) / 2;
+    static constexpr bool kDupClass = (g & 1) != 0;  // the antipodal class {p, p+g} is computed by both roles
+
+    // ---- shared-memory layout of one cell (in doubles; the cell index is the fastest dimension, stride CW) ----
+    // One table, row p = circle position p (rows 0..C-1, row C = a copy of row 0 for role 1's rotated reads):
+    //     col d = 0..g : X[p][p+d]      col g+1 : X[z][p]      col g+2 : w[p] = sqrt(eps_p)      col g+3 : 1 / w[p]
+    // then X[z][z], once per role (each role reads and writes its own copy through its shifted base pointer).
+    static constexpr int ROW = g + 4;
+    static constexpr int CZ = g + 1, CWT = g + 2, CIW = g + 3;
+    static constexpr int ZZ = (C + 1) * ROW;      // role 0's copy; role 1's is one row further
+    static constexpr int CELL = ZZ + ROW + 1;     // doubles per cell
+    // Horner-phase scratch (dead before the first matrix store): cols 0, 1 of row p
+    static constexpr int CAL = 0;                 // alpha[p] 2^-s
+    static constexpr int CBE = 1;                 // beta[p] 2^-s
+
+    static constexpr size_t kWarpBytes = (size_t)CELL * CW * sizeof(double);
+
+    __host__ __device__ static constexpr int md(int x) { return ((x % C) + C) % C; }
+    // slot of the pair of circle positions {p, q} (role-0 coordinates); the antipodal pair has a second slot
+    __host__ __device__ static constexpr int slot(int p, int q) {
+        const int d = md(q - p);
+        return d <= g ? p * ROW + d : q * ROW + (C - d);
+    }
+    __host__ __device__ static constexpr int slot2(int p, int q) { return md(q - p) == g ? q * ROW + g : -1; }
+    __host__ __device__ static constexpr int tix(int a, int b) { return a * g - (a * (a + 1)) / 2 + (b - a - 1); }
+    __host__ __device__ static constexpr int opos(int b) { return md(2 * b + 1); }  // other position b, role 0
+
+    // fp64-pipe instructions of one Horner step and one squaring per lane: prices the polynomial in choose_m_s
+    static constexpr int kHornerOps = NT + g * D + 4 * g + 3;
+    static constexpr int kSquareOps = n * (NT + g * D + g) + 2 * (NT + g * D + g) + 3 * g;
+    __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
+
+    // The last squaring is left out and X_{s-1} applied twice (a squaring is ~n^3/2 FMAs, an apply 3 n^2).
+    static constexpr int kDefer = 1;
+
+    struct Acc {  // the off-diagonal entries one lane computes
+        double T[NT > 0 ? NT : 1];
+        double M[g][D];
+        double Z[g];
+    };
+
+    // Byte offsets (from a lane's base pointer) of the n operands of every row l of a squaring, l = 0..C-1 the circle
+    // positions and l = C the gas row: sq[l][2a] = X[l][own a], sq[l][2a+1] = X[l][other a], sq[l][C] = X[l][z].
+    // The squaring loops over l with this table in constant memory: the loop body is 68 FMAs + 17 loads whatever l,
+    // 2 KB of code instead of the 29 KB of the unrolled form (which did not fit the 32 KB instruction cache next to
+    // the other phases: 18 % of the squaring's issue slots went to instruction fetch, ncu round 2).
+    struct Tab {
+        int sq[C + 1][C + 1];
+    };
+    __host__ __device__ static constexpr Tab make_tab() {
+        Tab t{};
+        for (int l = 0; l < C; ++l) {
+            for (int a = 0; a < g; ++a) {
+                t.sq[l][2 * a] = slot(l, 2 * a) * CW * 8;
+                t.sq[l][2 * a + 1] = slot(l, opos(a)) * CW * 8;
+            }
+            t.sq[l][C] = (l * ROW + CZ) * CW * 8;
+        }
+        for (int a = 0; a < g; ++a) {
+            t.sq[C][2 * a] = ((2 * a) * ROW + CZ) * CW * 8;
+            t.sq[C][2 * a + 1] = ((2 * a + 1) * ROW + CZ) * CW * 8;
+        }
+        t.sq[C][C] = ZZ * CW * 8;
+        return t;
+    }
+
+    // A lane's view of its cell: the base pointer with the role shift (one table row) folded in.
+    struct View {
+        double* x;
+        int r;
+    };
+    __device__ __forceinline__ static View view(double* warp_tile, int lane) {
+        const int r = lane >> 4, c = lane & 15;
+        View v;
+        v.x = warp_tile + c + r * ROW * CW;
+        v.r = r;
+        return v;
+    }
+    __device__ __forceinline__ static double& at(const View& V, int row, int col) { return V.x[(row * ROW + col) * CW]; }
+
+    __device__ __forceinline__ static double lds(const double* base, int byte_off) {
+        return *reinterpret_cast<const volatile double*>(reinterpret_cast<const char*>(base) + byte_off);
+    }
+
+    // ---- one squaring: A <- off-diagonals of X X (own share) -----------------------------------------------------
+    // volatile loads: every row is fetched when it is used.
+    template <bool First>
+    __device__ __forceinline__ static void square_row(const View& V, const int* off, Acc& A) {
+        double u[g], o[g];
+        static_for<0, g>([&](auto a) {
+            u[a] = lds(V.x, off[2 * a]);
+            o[a] = lds(V.x, off[2 * a + 1]);
+        });
+        const double z = lds(V.x, off[C]);
+        static_for<0, g>([&](auto a) {
+            static_for<a + 1, g>([&](auto b) {
+                if constexpr (First) A.T[tix(a, b)] = u[a] * u[b];
+                else A.T[tix(a, b)] = fma(u[a], u[b], A.T[tix(a, b)]);
+            });
+            static_for<0, D>([&](auto dd) {
+                if constexpr (First) A.M[a][dd] = u[a] * o[(a + dd) % g];
+                else A.M[a][dd] = fma(u[a], o[(a + dd) % g], A.M[a][dd]);
+            });
+            if constexpr (First) A.Z[a] = z * u[a];
+            else A.Z[a] = fma(z, u[a], A.Z[a]);
+        });
+    }
+    __device__ __forceinline__ static void square(const View& V, const Tab& tab, Acc& A) {
+        square_row<true>(V, tab.sq[0], A);
+#pragma unroll 1
+        for (int l = 1; l <= C; ++l) square_row<false>(V, tab.sq[l], A);
+    }
+
+    // ---- conservation + store ------------------------------------------------------------------------------------
+    // The diagonal from conservation of total momentum:  d_j = -(sum_{i != j} w_i O_ij) / w_j  (w_z = 1).  Every lane
+    // sums its own entries into the columns they touch; the partner's share of a lane's own columns comes by shuffle.
+    // Writes the off-diagonals, the diagonal (X_jj = 1 + d_j, or d_j itself when `fin`: the matrix handed to the apply
+    // step is P = X - I) and the copies the rotated addressing needs.  `active` = this cell still takes part.
+    __device__ __forceinline__ static void conserve_store(const View& V, const Acc& A, bool active, bool fin) {
+        const int r = V.r;
+        double cu[g], co[g], cz = 0.0;
+        double wu[g], wo[g];
+        static_for<0, g>([&](auto a) {
+            wu[a] = at(V, 2 * a, CWT);
+            wo[a] = at(V, 2 * a + 1, CWT);
+            cu[a] = 0.0;
+            co[a] = 0.0;
+        });
+        static_for<0, g>([&](auto a) {
+            static_for<a + 1, g>([&](auto b) {
+                const double v = A.T[tix(a, b)];
+                cu[a] = fma(wu[b], v, cu[a]);
+                cu[b] = fma(wu[a], v, cu[b]);
+            });
+            static_for<0, D>([&](auto dd) {
+                constexpr int b = (a + dd) % g;
+                double v = A.M[a][dd];
+                if constexpr (kDupClass && dd == D - 1) v = r ? 0.0 : v;  // counted by role 0 only
+                cu[a] = fma(wo[b], v, cu[a]);
+                co[b] = fma(wu[a], v, co[b]);
+            });
+            cu[a] += A.Z[a];
+            cz = fma(wu[a], A.Z[a], cz);
+        });
+        // partner's sums for MY own columns: its other-position b is my own position a = b + 1 - r_partner
+        double dgl[g];
+        static_for<0, g>([&](auto b) { co[b] = __shfl_xor_sync(0xffffffffu, co[b], 16); });
+        static_for<0, g>([&](auto a) {
+            const double pv = r ? co[a] : co[(a + g - 1) % g];
+            const double d = -(cu[a] + pv) * at(V, 2 * a, CIW);
+            dgl[a] = fin ? d : 1.0 + d;
+        });
+        {
+            const double other = __shfl_xor_sync(0xffffffffu, cz, 16);
+            const double lo = r ? other : cz, hi = r ? cz : other;  // same order in both lanes
+            cz = -(lo + hi);
+            cz = fin ? cz : 1.0 + cz;
+        }
+        __syncwarp();  // every lane has finished reading the old matrix (or the Horner scratch)
+        if (active) {
+            const bool r0 = (r == 0);
+            static_for<0, g>([&](auto a) {
+                static_for<a + 1, g>([&](auto b) {
+                    constexpr int s1 = slot(2 * a, 2 * b), s2 = slot2(2 * a, 2 * b);
+                    const double v = A.T[tix(a, b)];
+                    V.x[s1 * CW] = v;
+                    if constexpr (s2 >= 0) V.x[s2 * CW] = v;
+                    if constexpr (s1 / ROW == 0)
+                        if (r0) V.x[(s1 + C * ROW) * CW] = v;  // row C = copy of row 0 (row 0 belongs to role 0)
+                });
+                static_for<0, D>([&](auto dd) {
+                    constexpr int q = opos((a + dd) % g);
+                    constexpr int s1 = slot(2 * a, q), s2 = slot2(2 * a, q);
+                    const double v = A.M[a][dd];
+                    if constexpr (kDupClass && dd == D - 1) {  // antipodal class: role 0 stores both slots
+                        if (r0) {
+                            V.x[s1 * CW] = v;
+                            V.x[s2 * CW] = v;
+                            if constexpr (s1 / ROW == 0) V.x[(s1 + C * ROW) * CW] = v;
+                            if constexpr (s2 / ROW == 0) V.x[(s2 + C * ROW) * CW] = v;
+                        }
+                    } else {
+                        V.x[s1 * CW] = v;
+                        if constexpr (s2 >= 0) V.x[s2 * CW] = v;
+                        if constexpr (s1 / ROW == 0)
+                            if (r0) V.x[(s1 + C * ROW) * CW] = v;
+                    }
+                });
+                at(V, 2 * a, CZ) = A.Z[a];
+                at(V, 2 * a, 0) = dgl[a];
+                if constexpr (a == 0) {
+                    if (r0) {
+                        at(V, C, CZ) = A.Z[a];
+                        at(V, C, 0) = dgl[a];
+                    }
+                }
+            });
+            V.x[ZZ * CW] = cz;  // each role its own copy
+        }
+        __syncwarp();
+    }
+
+    // ---- Taylor polynomial T_m(S / 2^s) - I  (Eq. 19), factored Horner recurrence of dg_tpc.cuh ----------------------
+    // Q_j = (m!/j!) P_j,  Q_0k = beta_k v_k,  Q_ik = beta_i beta_k U_ik:
+    //     U_ik <- v_k - alpha_i U_ik,   v_k <- (kappa_j + Q_00) - alpha_k v_k,   Q_00 <- b00 (kappa_j + Q_00) + sum_l beta_l^2 v_l
+    // (right-hand sides: old values).  The lane owns U for its pairs (T: own a, own b; M: own a, other b) and carries
+    // v at all C positions (its own and the other role's: 2 g FMAs more per step, no cross-lane traffic in the loop).
+    // For an M pair the recurrence is used in its mirrored form U <- v_own - alpha_other U (B Q is symmetric).
+    // alpha, beta (already scaled by 2^-s) are read from the Horner scratch in shared memory.  m is warp-uniform.
+    __device__ __forceinline__ static void horner(const View& V, int m, double b00, Acc& A) {
+        double alu[g], alo[g], b2u[g], b2o[g], vu[g], vo[g];
+        static_for<0, g>([&](auto a) {
+            alu[a] = at(V, 2 * a, CAL);
+            alo[a] = at(V, 2 * a + 1, CAL);
+            const double bu = at(V, 2 * a, CBE), bo = at(V, 2 * a + 1, CBE);
+            b2u[a] = bu * bu;
+            b2o[a] = bo * bo;
+            vu[a] = 1.0;
+            vo[a] = 1.0;
+            static_for<0, D>([&](auto dd) { A.M[a][dd] = 0.0; });
+        });
+        static_for<0, (NT > 0 ? NT : 1)>([&](auto K) { A.T[K] = 0.0; });
+        double q00 = b00, kap = 1.0;
+        for (int j = m - 1; j >= 1; --j) {
+            kap *= c_dbl[j + 1];
+            static_for<0, g>([&](auto a) {
+                static_for<a + 1, g>([&](auto b) { A.T[tix(a, b)] = fma(-alu[a], A.T[tix(a, b)], vu[b]); });
+                static_for<0, D>([&](auto dd) {
+                    constexpr int b = (a + dd) % g;
+                    A.M[a][dd] = fma(-alo[b], A.M[a][dd], vu[a]);
+                });
+            });
+            double t00 = b2u[0] * vu[0];
+            static_for<1, g>([&](auto a) { t00 = fma(b2u[a], vu[a], t00); });
+            static_for<0, g>([&](auto a) { t00 = fma(b2o[a], vo[a], t00); });
+            const double x00 = kap + q00;
+            static_for<0, g>([&](auto a) {
+                vu[a] = fma(-alu[a], vu[a], x00);
+                vo[a] = fma(-alo[a], vo[a], x00);
+            });
+            q00 = fma(b00, x00, t00);
+        }
+        // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!; off-diagonals are >= 0 in exact arithmetic
+        const double inv = c_ifact[m];
+        static_for<0, g>([&](auto a) {
+            const double bs = at(V, 2 * a, CBE) * inv;
+            A.Z[a] = clamp_below(bs * vu[a], 0.0);
+            static_for<a + 1, g>([&](auto b) {
+                A.T[tix(a, b)] = clamp_below(A.T[tix(a, b)] * (bs * at(V, 2 * b, CBE)), 0.0);
+            });
+            static_for<0, D>([&](auto dd) {
+                constexpr int b = (a + dd) % g;
+                A.M[a][dd] = clamp_below(A.M[a][dd] * (bs * at(V, 2 * b + 1, CBE)), 0.0);
+            });
+        });
+    }
+
+    // ---- apply: y = P q for this lane's rows (its own positions) and the gas row ------------------------------------
+    // q[comp][j] (j = 0..C-1 in role-rotated order: index j <-> position j + r) and q0[comp] are the three W^-1 p_in
+    // vectors; row(a, y) receives the result row at the own position a (three components), y0[comp] is the gas row
+    // (computed by both lanes).
+    template <class RowFn>
+    __device__ __forceinline__ static void apply(const View& V, const double (&q)[3][C], const double (&q0)[3],
+                                                 double (&y0)[3], RowFn&& row) {
+        {
+            const double dz = V.x[ZZ * CW];
+            static_for<0, 3>([&](auto cp) { y0[cp] = dz * q0[cp]; });
+            static_for<0, C>([&](auto j) {
+                const double e = at(V, j, CZ);  // X[z][position j + r]
+                static_for<0, 3>([&](auto cp) { y0[cp] = fma(e, q[cp][j], y0[cp]); });
+            });
+        }
+        static_for<0, g>([&](auto a) {
+            const double ez = at(V, 2 * a, CZ);
+            double acc[3];
+            static_for<0, 3>([&](auto cp) { acc[cp] = ez * q0[cp]; });
+            static_for<0, C>([&](auto j) {
+                const double e = V.x[slot(2 * a, j) * CW];  // X[own position a][position j + r] (j = 2a: the diagonal d)
+                static_for<0, 3>([&](auto cp) { acc[cp] = fma(e, q[cp][j], acc[cp]); });
+            });
+            row(a, acc);
+        });
+    }
+};
+
+}  // namespace dg

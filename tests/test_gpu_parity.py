@@ -77,11 +77,11 @@ def test_sweep_every_species_count(dg, oracle, cuda, N):
     run_and_compare(dg, oracle, wl)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 4])
 @pytest.mark.parametrize("N", list(range(1, 17)))
 def test_both_thread_mappings_for_every_species_count(dg, oracle, cuda, N, variant):
-    """dg_drag_update_variant: thread-per-cell (1) and warp-per-cell DMMA (2) each against the oracle, for every N,
-    on the stiff configs[4] generator and on the Dustywave-like configs[2] recipe."""
+    """dg_drag_update_variant: thread-per-cell (1), warp-per-cell DMMA (2) and pair-per-cell (4) each against the
+    oracle, for every N, on the stiff configs[4] generator and on the Dustywave-like configs[2] recipe."""
     wl = W.make_workload(5, ncells=700 + 13 * N, N=N, device=cuda)
     run_and_compare(dg, oracle, wl, variant=variant)
     wl = W.make_workload(3, ncells=333, N=N, device=cuda)
@@ -269,7 +269,7 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
     from mpmath import mp, mpf
     mp.dps = 90
     wl = _extreme_workload(N, cuda)
-    variants = (0,) if N < 8 else (0, 1, 2)
+    variants = (0,) if N < 8 else (0, 1, 2, 4)
     outs = {v: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=v) for v in variants}
     rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(wl.ncells))
     n = N + 1
@@ -292,7 +292,7 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
                     assert abs(mpf(float(o[comp, k])) - refs[comp][k]) <= PARITY_TOL * scale, (N, c, v, comp, k)
 
 
-@pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0)])
+@pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0), (16, 4), (7, 4)])
 @pytest.mark.parametrize("ncells", [512, 515, 2050])
 def test_pointers_that_are_8_but_not_16_byte_aligned(dg, oracle, cuda, N, variant, ncells):
     """include/dg.h asks for 8-byte alignment only.  Every array is a view starting one double into its allocation
@@ -326,7 +326,7 @@ def test_pointers_that_are_8_but_not_16_byte_aligned(dg, oracle, cuda, N, varian
 
 
 @pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])
 def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
     """include/dg.h: non-finite input gives non-finite output in that cell only.  With the thread-per-cell mapping
     the poisoned cell shares a warp (and the warp's Taylor degree, R8) with 31 healthy ones: they must still
@@ -361,7 +361,7 @@ def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
     n = N + 1
     guard = 4096
     size = 3 * n * ncells
-    for which in ("tpc", "wpc", "paper", "rk1", "steps"):
+    for which in ("tpc", "wpc", "ppc", "paper", "rk1", "steps"):
         big = torch.full((size + 2 * guard,), -7.25, dtype=torch.float64, device=cuda)
         p_out = big[guard:guard + size].view(3, n, ncells)
         if which == "rk1":
@@ -369,7 +369,7 @@ def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
         elif which == "steps":
             dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 3, p_out=p_out)
         else:
-            variant = {"tpc": 1, "wpc": 2, "paper": 3}[which]
+            variant = {"tpc": 1, "wpc": 2, "paper": 3, "ppc": 4}[which]
             dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=variant)
         torch.cuda.synchronize()
         assert bool((big[:guard] == -7.25).all()) and bool((big[guard + size:] == -7.25).all()), which
