@@ -131,31 +131,45 @@ struct Ppc {
 
     // ---- one squaring: A <- off-diagonals of X X (own share) -----------------------------------------------------
     // volatile loads: every row is fetched when it is used.
-    template <bool First>
-    __device__ __forceinline__ static void square_row(const View& V, const int* off, Acc& A) {
-        double u[g], o[g];
+    struct RowOps {  // the n operands of one row l
+        double u[g], o[g], z;
+    };
+    __device__ __forceinline__ static void load_row(const View& V, const int* off, RowOps& R) {
         static_for<0, g>([&](auto a) {
-            u[a] = lds(V.x, off[2 * a]);
-            o[a] = lds(V.x, off[2 * a + 1]);
+            R.u[a] = lds(V.x, off[2 * a]);
+            R.o[a] = lds(V.x, off[2 * a + 1]);
         });
-        const double z = lds(V.x, off[C]);
+        R.z = lds(V.x, off[C]);
+    }
+    template <bool First>
+    __device__ __forceinline__ static void fma_row(const RowOps& R, Acc& A) {
         static_for<0, g>([&](auto a) {
             static_for<a + 1, g>([&](auto b) {
-                if constexpr (First) A.T[tix(a, b)] = u[a] * u[b];
-                else A.T[tix(a, b)] = fma(u[a], u[b], A.T[tix(a, b)]);
+                if constexpr (First) A.T[tix(a, b)] = R.u[a] * R.u[b];
+                else A.T[tix(a, b)] = fma(R.u[a], R.u[b], A.T[tix(a, b)]);
             });
             static_for<0, D>([&](auto dd) {
-                if constexpr (First) A.M[a][dd] = u[a] * o[(a + dd) % g];
-                else A.M[a][dd] = fma(u[a], o[(a + dd) % g], A.M[a][dd]);
+                if constexpr (First) A.M[a][dd] = R.u[a] * R.o[(a + dd) % g];
+                else A.M[a][dd] = fma(R.u[a], R.o[(a + dd) % g], A.M[a][dd]);
             });
-            if constexpr (First) A.Z[a] = z * u[a];
-            else A.Z[a] = fma(z, u[a], A.Z[a]);
+            if constexpr (First) A.Z[a] = R.z * R.u[a];
+            else A.Z[a] = fma(R.z, R.u[a], A.Z[a]);
         });
     }
+    // Rows 0..C (C + 1 of them, an odd number), two per loop iteration with the operands double-buffered: the loads of
+    // the next row are in flight while the FMAs of the current one issue.
     __device__ __forceinline__ static void square(const View& V, const Tab& tab, Acc& A) {
-        square_row<true>(V, tab.sq[0], A);
+        RowOps Ra, Rb;
+        load_row(V, tab.sq[0], Ra);
+        load_row(V, tab.sq[1], Rb);
+        fma_row<true>(Ra, A);
 #pragma unroll 1
-        for (int l = 1; l <= C; ++l) square_row<false>(V, tab.sq[l], A);
+        for (int l = 1; l < C; l += 2) {
+            load_row(V, tab.sq[l + 1], Ra);
+            fma_row<false>(Rb, A);
+            load_row(V, tab.sq[l + 2 <= C ? l + 2 : C], Rb);  // (the last iteration re-reads row C: never used)
+            fma_row<false>(Ra, A);
+        }
     }
 
     // ---- conservation + store ------------------------------------------------------------------------------------

@@ -37,30 +37,58 @@ constexpr size_t kSmemBytes = kMatBytes + sizeof(unsigned short) * kTile + 16;
 
 __constant__ const Core::Tab c_tab = Core::make_tab();
 
-// Norm bound  max_i a_i + sum_i eps_i a_i  (R5) -> sort key: stiffest first, non-finite first of all.
-__device__ __forceinline__ unsigned sort_key(const UpdateArgs& G, int N, long long cell, bool ok) {
-    const long long nc = G.ncells;
-    double ts[NP], rd[NP];
-    const double rg = ok ? __ldg(G.rho_g + cell) : 1.0;
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {  // all loads first: one round trip, not N
-        const bool live = ok && i < N;
-        ts[i] = live ? __ldg(G.t_s + (long long)i * nc + cell) : 1.0;
-        rd[i] = live ? __ldg(G.rho_d + (long long)i * nc + cell) : 0.0;
-    }
-    const double irg = fast_rcp(rg);
-    double sb = 0.0, amax = 0.0;
-#pragma unroll
-    for (int i = 0; i < NP; ++i) {
-        const double a = (i < N) ? G.dt * fast_rcp(ts[i]) : 0.0;
-        sb = fma(rd[i] * irg, a, sb);
-        amax = fmax(amax, a);
-    }
-    const unsigned e = ((unsigned)__double2hiint(sb + amax) >> 20) & 0x7ffu;  // biased exponent (0x7ff: Inf / NaN)
-    return ok ? 0x7ffu - e : 0xfffu;
-}
-
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// A load the compiler may not sink towards its first use: the gathers of a chunk are issued back to back (one round
+// trip to L2 / HBM for all of them), not one per dependent reciprocal.
+__device__ __forceinline__ double ldg_now(const double* p) {
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+// Emits nothing; placed after a batch of ldg_now() it keeps every use of v behind the LAST load of the batch (volatile
+// asm statements keep their order), so that no dependent instruction stalls the warp before all loads have been issued.
+__device__ __forceinline__ void after_loads(double& v) { asm volatile("" : "+d"(v)); }
+
+// Sort keys of the kPerThread cells base + threadIdx.x + j kThreads: the binary exponent of the norm bound
+// max_i a_i + sum_i eps_i a_i (R5), stiffest first, non-finite first of all; cells past the end last.
+// Species-major so that the loads of all the thread's cells for one species are in flight together.
+__device__ __forceinline__ void sort_keys(const UpdateArgs& G, int N, long long base, int count, unsigned* keys) {
+    const long long nc = G.ncells;
+    long long cell[kPerThread];
+    double irg[kPerThread], sb[kPerThread], amax[kPerThread];
+#pragma unroll
+    for (int j = 0; j < kPerThread; ++j) {
+        const int idx = threadIdx.x + j * kThreads;
+        cell[j] = base + (idx < count ? idx : 0);
+        irg[j] = ldg_now(G.rho_g + cell[j]);
+        sb[j] = 0.0;
+        amax[j] = 0.0;
+    }
+#pragma unroll
+    for (int j = 0; j < kPerThread; ++j) irg[j] = fast_rcp(irg[j]);
+#pragma unroll 2
+    for (int i = 0; i < N; ++i) {
+        double ts[kPerThread], rd[kPerThread];
+#pragma unroll
+        for (int j = 0; j < kPerThread; ++j) {
+            ts[j] = ldg_now(G.t_s + (long long)i * nc + cell[j]);
+            rd[j] = ldg_now(G.rho_d + (long long)i * nc + cell[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < kPerThread; ++j) {
+            const double a = G.dt * fast_rcp(ts[j]);
+            sb[j] = fma(rd[j] * irg[j], a, sb[j]);
+            amax[j] = fmax(amax[j], a);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < kPerThread; ++j) {
+        const int idx = threadIdx.x + j * kThreads;
+        const unsigned e = ((unsigned)__double2hiint(sb[j] + amax[j]) >> 20) & 0x7ffu;  // 0x7ff: Inf / NaN
+        const unsigned key = (idx < count) ? 0x7ffu - e : 0xfffu;
+        keys[idx] = (key << 16) | (unsigned)idx;
+    }
+}
 
 __device__ __forceinline__ void sort_tile(unsigned* keys) {
 #pragma unroll 1
@@ -101,12 +129,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
         const long long base = tile * kTile;
         const int count = (nc - base < kTile) ? (int)(nc - base) : kTile;
         // ---- 1. sort the tile by stiffness
-#pragma unroll 2
-        for (int j = 0; j < kPerThread; ++j) {
-            const int idx = threadIdx.x + j * kThreads;
-            const unsigned key = sort_key(G, N, base + idx, idx < count);
-            keys[idx] = (key << 16) | (unsigned)idx;
-        }
+        sort_keys(G, N, base, count, keys);
         if (threadIdx.x == 0) *next_chunk = 0;
         __syncthreads();
         // (a tile whose cells all carry one key is already in order)
@@ -128,11 +151,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
         const int nchunks = (count + CW - 1) / CW;
 
         // ---- 2. chunks of 16 sorted cells
-        for (;;) {
+        auto claim = [&]() {
             int j = 0;
             if (lane == 0) j = atomicAdd(next_chunk, 1);
-            j = __shfl_sync(kFullMask, j, 0);
-            if (j >= nchunks) break;
+            return __shfl_sync(kFullMask, j, 0);
+        };
+        int jnext = claim();
+        while (jnext < nchunks) {
+            const int j = jnext;
+            jnext = claim();  // the chunk after this one (its fields are prefetched into L2 before this one's apply step)
             const int pos = j * CW + c;
             const bool valid = pos < count;
             const long long cell = base + (valid ? (int)order[pos] : 0);
@@ -142,30 +169,25 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             double sbp = 0.0, amx = 0.0;
             {
                 double ts[g], rd[g];
-                const double rg = valid ? __ldg(G.rho_g + cell) : 1.0;
+                const double rg = ldg_now(G.rho_g + cell);  // (an absent cell reads the tile's first cell)
                 static_for<0, g>([&](auto a) {  // all loads first: one round trip
-                    const int k = 2 * a + r;    // dust species at my own position a
-                    const bool live = valid && k < N;
-                    ts[a] = live ? __ldg(G.t_s + (long long)k * nc + cell) : 1.0;
-                    rd[a] = live ? __ldg(G.rho_d + (long long)k * nc + cell) : 1.0;
+                    const int k = 2 * a + r;    // dust species at my own position a (an inert slot re-reads species 0)
+                    const long long row = (long long)(k < N ? k : 0) * nc + cell;
+                    ts[a] = ldg_now(G.t_s + row);
+                    rd[a] = ldg_now(G.rho_d + row);
                 });
-                // the momenta are needed after the squarings: start them on their way to L2 / L1 now
-                if (valid) {
-                    static_for<0, 3>([&](auto cp) {
-                        static_for<0, g>([&](auto a) {
-                            const int k = 2 * a + r;
-                            if (k < N) prefetch_l2(G.p_in + ((long long)cp * n + 1 + k) * nc + cell);
-                        });
-                        if (r == 0) prefetch_l2(G.p_in + ((long long)cp * n) * nc + cell);
-                    });
-                }
+                static_for<0, g>([&](auto a) {
+                    after_loads(ts[a]);
+                    after_loads(rd[a]);
+                });
                 const double irg = fast_rcp(rg);
                 static_for<0, g>([&](auto a) {
                     const int k = 2 * a + r;
                     const bool live = valid && k < N;
                     double w, iw;
                     sym_weights(rd[a] * irg, w, iw);
-                    const double aa = live ? G.dt * fast_rcp(ts[a]) : 0.0;
+                    double aa = G.dt * fast_rcp(ts[a]);
+                    aa = live ? aa : 0.0;
                     w = live ? w : 1.0;
                     iw = live ? iw : 1.0;
                     av[a] = aa;
@@ -210,13 +232,41 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             const int napply = 1 << min(Core::kDefer, s);
             Core::conserve_store(V, A, true, nsq == 0);
             const int smax = __reduce_max_sync(kFullMask, nsq);
+            // Prefetches into L2, issued one phase ahead of their use — early enough to cover the HBM latency, late enough
+            // that the lines are still there (the tiles in flight on all SMs are larger than L2): this cell's momenta
+            // before the last squaring, the next chunk's fields before the apply step.
+            auto prefetch_momenta = [&]() {
+                if (valid) {
+                    static_for<0, 3>([&](auto cp) {
+                        static_for<0, g>([&](auto a) {
+                            const int k = 2 * a + r;
+                            if (k < N) prefetch_l2(G.p_in + ((long long)cp * n + 1 + k) * nc + cell);
+                        });
+                        if (r == 0) prefetch_l2(G.p_in + ((long long)cp * n) * nc + cell);
+                    });
+                }
+            };
+            if (smax == 0) prefetch_momenta();
             for (int it = 0; it < smax; ++it) {
+                if (it == smax - 1) prefetch_momenta();
                 Core::square(V, c_tab, A);
                 Core::conserve_store(V, A, it < nsq, it == nsq - 1);
             }
             if (valid && r == 0) {
                 if (G.s_out) G.s_out[cell] = s;
                 if (G.m_out) G.m_out[cell] = m;
+            }
+
+            if (jnext < nchunks && jnext * CW + c < count) {
+                const long long cn = base + (int)order[jnext * CW + c];
+                if (r == 0) prefetch_l2(G.rho_g + cn);
+                static_for<0, g>([&](auto a) {
+                    const int k = 2 * a + r;
+                    if (k < N) {
+                        prefetch_l2(G.t_s + (long long)k * nc + cn);
+                        prefetch_l2(G.rho_d + (long long)k * nc + cn);
+                    }
+                });
             }
 
             // a5: p_out = p_in + W P W^-1 p_in (Eq. 18), applied 2^min(defer, s) times
