@@ -77,8 +77,8 @@ struct Ppc {
     static constexpr int kSquareOps = n * (NT + g * D + g) + 2 * (NT + g * D + g) + 3 * g;
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
-    // The last squaring is left out and X_{s-1} applied twice (a squaring is ~n^3/2 FMAs, an apply 3 n^2).
-    static constexpr int kDefer = 1;
+    // (No "apply X_{s-1} twice instead of the last squaring" here, unlike dg_tpc.cuh for N = 6..10: with the iterate in
+    // shared memory a second apply costs this mapping as much time as the squaring it would save — measured.)
 
     struct Acc {  // the off-diagonal entries one lane computes
         double T[NT > 0 ? NT : 1];
@@ -91,8 +91,12 @@ struct Ppc {
     // The squaring loops over l with this table in constant memory: the loop body is 68 FMAs + 17 loads whatever l,
     // 2 KB of code instead of the 29 KB of the unrolled form (which did not fit the 32 KB instruction cache next to
     // the other phases: 18 % of the squaring's issue slots went to instruction fetch, ncu round 2).
+    // ap[a][j]: the operands of row a of the apply step, a = 0..g-1 the lane's own positions and a = g the gas row:
+    // ap[a][j] = X[own a][position j], j = 0..C-1 (j = 2a: the diagonal), ap[a][C] = X[own a][z]; for the gas row
+    // ap[g][j] = X[z][position j], ap[g][C] = X[z][z].
     struct Tab {
         int sq[C + 1][C + 1];
+        int ap[g + 1][C + 1];
     };
     __host__ __device__ static constexpr Tab make_tab() {
         Tab t{};
@@ -108,6 +112,12 @@ struct Ppc {
             t.sq[C][2 * a + 1] = ((2 * a + 1) * ROW + CZ) * CW * 8;
         }
         t.sq[C][C] = ZZ * CW * 8;
+        for (int a = 0; a < g; ++a) {
+            for (int j = 0; j < C; ++j) t.ap[a][j] = slot(2 * a, j) * CW * 8;
+            t.ap[a][C] = ((2 * a) * ROW + CZ) * CW * 8;
+        }
+        for (int j = 0; j < C; ++j) t.ap[g][j] = (j * ROW + CZ) * CW * 8;
+        t.ap[g][C] = ZZ * CW * 8;
         return t;
     }
 
@@ -316,31 +326,26 @@ struct Ppc {
         });
     }
 
-    // ---- apply: y = P q for this lane's rows (its own positions) and the gas row ------------------------------------
+    // ---- apply: one row of y = P q ---------------------------------------------------------------------------------
     // q[comp][j] (j = 0..C-1 in role-rotated order: index j <-> position j + r) and q0[comp] are the three W^-1 p_in
-    // vectors; row(a, y) receives the result row at the own position a (three components), y0[comp] is the gas row
-    // (computed by both lanes).
-    template <class RowFn>
-    __device__ __forceinline__ static void apply(const View& V, const double (&q)[3][C], const double (&q0)[3],
-                                                 double (&y0)[3], RowFn&& row) {
-        {
-            const double dz = V.x[ZZ * CW];
-            static_for<0, 3>([&](auto cp) { y0[cp] = dz * q0[cp]; });
-            static_for<0, C>([&](auto j) {
-                const double e = at(V, j, CZ);  // X[z][position j + r]
-                static_for<0, 3>([&](auto cp) { y0[cp] = fma(e, q[cp][j], y0[cp]); });
-            });
-        }
-        static_for<0, g>([&](auto a) {
-            const double ez = at(V, 2 * a, CZ);
-            double acc[3];
-            static_for<0, 3>([&](auto cp) { acc[cp] = ez * q0[cp]; });
-            static_for<0, C>([&](auto j) {
-                const double e = V.x[slot(2 * a, j) * CW];  // X[own position a][position j + r] (j = 2a: the diagonal d)
-                static_for<0, 3>([&](auto cp) { acc[cp] = fma(e, q[cp][j], acc[cp]); });
-            });
-            row(a, acc);
+    // vectors; `off` = tab.ap[row].  Returns y[comp] = P[row][z] q0 + sum_j P[row][j] q_j.  Two partial sums per
+    // component (six independent FMA chains).  The caller loops over the rows: the code is the same for every row.
+    __device__ __forceinline__ static void apply_row(const View& V, const int* off, const double (&q)[3][C],
+                                                     const double (&q0)[3], double (&y)[3]) {
+        double e[C + 1];
+        static_for<0, C + 1>([&](auto j) { e[j] = lds(V.x, off[j]); });
+        double ya[3], yb[3];
+        static_for<0, 3>([&](auto cp) {
+            ya[cp] = e[C] * q0[cp];
+            yb[cp] = e[0] * q[cp][0];
         });
+        static_for<1, C>([&](auto j) {
+            static_for<0, 3>([&](auto cp) {
+                if constexpr (j % 2 == 1) ya[cp] = fma(e[j], q[cp][j], ya[cp]);
+                else yb[cp] = fma(e[j], q[cp][j], yb[cp]);
+            });
+        });
+        static_for<0, 3>([&](auto cp) { y[cp] = ya[cp] + yb[cp]; });
     }
 };
 

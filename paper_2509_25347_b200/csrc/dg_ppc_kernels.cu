@@ -1,16 +1,22 @@
 // dg_ppc_kernels.cu — pair-per-cell fused kernel for NP = DG_NP dust slots (NP even; serves N = NP and N = NP - 1, the
 // odd count running with one inert slot: a = 0, w = 1).  Core and layout: dg_ppc.cuh.
 //
-// One block per SM, 8 warps; a warp works on CHUNKS of 16 cells (two lanes per cell), the cell's matrix in the warp's
-// private shared-memory tile.  Cells are handed out in TILES of kTile consecutive cells:
-//   1. the block computes the norm bound of every cell of the tile (the fields are read once more for this: 33 of the
-//      84 doubles a cell moves, from L2 the second time) and sorts the tile by the norm's binary exponent, stiffest
-//      first (bitonic sort on (key, cell) words: deterministic);
-//   2. warps claim chunks of 16 sorted cells from a shared counter.  The lanes of a warp run the largest s and the common
-//      Taylor degree m of their 16 cells (R8), so after the sort a chunk holds cells of (nearly) one s and
-//      nothing is executed for lanes that are already done — the divergence Alg. 2 is written to avoid.
-// Loads and stores of the fields are therefore gathers inside a 2048-cell window (16 KB per field row, L1/L2-resident);
-// at N >= 13 the kernel is bound by the fp64 pipe by a factor of ~20 over HBM, so the gathers do not show.
+// One block per SM, 8 warps; a warp works on CHUNKS of 16 cells (two lanes per cell), the cells' matrices in the warp's
+// private shared-memory tile.  The lanes of a warp run the largest s and the common Taylor degree m of their 16 cells
+// (R8), so cells are handed out sorted by stiffness — the divergence Alg. 2 is written to avoid
+// (PAPER.md:646):
+//   * the block walks TILES of kTile consecutive cells (tile k of block b is tile b + k gridDim.x of the array);
+//   * ONE warp sorts a tile: it computes the norm bound of every cell (reading the 2N + 1 field rows of the tile,
+//     coalesced) and sorts (key, cell) words, stiffest first, with a bitonic network in its own shared-memory tile —
+//     deterministic, no block barrier;
+//   * all warps claim chunks of 16 sorted cells from the tile's counter; the warp that claims the FIRST chunk of tile k
+//     sorts tile k + 1 before it starts on its chunk, so the next tile is ready long before this one runs out
+//     (three order buffers: the one being overwritten belongs to tile k - 2).  No warp ever waits for another one
+//     except at the very start.
+// Loads and stores of the fields are gathers inside a tile.  A tile is small (256 cells, 172 KB of fields) so that the
+// tiles in flight on all SMs stay L2-resident: with 2048-cell tiles they did not (5.6 KB of DRAM reads per cell for
+// 0.94 KB needed, ncu round 2), because a 32-byte sector fetched for one cell was evicted before its three neighbours
+// were processed.
 #include "dg_internal.h"
 #include "dg_ppc.cuh"
 
@@ -26,159 +32,210 @@ using Core = Ppc<NP>;
 constexpr int C = Core::C, g = Core::g, CW = Core::CW;
 constexpr int kWarps = 8;
 constexpr int kThreads = 32 * kWarps;
-constexpr int kTile = 2048;
-constexpr int kPerThread = kTile / kThreads;
+constexpr int kTile = 256;
+constexpr int kPerLane = kTile / 32;
+constexpr int kBufs = 3;
 constexpr unsigned kFullMask = 0xffffffffu;
 
+struct Sched {  // block-wide scheduling state
+    unsigned short order[kBufs][kTile];  // sorted cell offsets of the tiles in flight
+    int next[kBufs];                     // chunk claim counter
+    int ready[kBufs];                    // sequence number of the tile whose order is in the buffer (-1: none)
+};
 constexpr size_t kTilesBytes = Core::kWarpBytes * kWarps;
-constexpr size_t kSortBytes = sizeof(unsigned) * kTile;  // aliases the warp tiles (idle while the block sorts)
-constexpr size_t kMatBytes = kTilesBytes > kSortBytes ? kTilesBytes : kSortBytes;
-constexpr size_t kSmemBytes = kMatBytes + sizeof(unsigned short) * kTile + 16;
+static_assert(Core::kWarpBytes >= sizeof(unsigned) * kTile, "a warp sorts a tile inside its own shared-memory tile");
+constexpr size_t kSmemBytes = kTilesBytes + sizeof(Sched);
 
 __constant__ const Core::Tab c_tab = Core::make_tab();
 
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-// A load the compiler may not sink towards its first use: the gathers of a chunk are issued back to back (one round
-// trip to L2 / HBM for all of them), not one per dependent reciprocal.
+// A load the compiler's front end may not sink towards its first use (the sort keys: all loads of a species together).
 __device__ __forceinline__ double ldg_now(const double* p) {
     double v;
     asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
-// Emits nothing; placed after a batch of ldg_now() it keeps every use of v behind the LAST load of the batch (volatile
-// asm statements keep their order), so that no dependent instruction stalls the warp before all loads have been issued.
-__device__ __forceinline__ void after_loads(double& v) { asm volatile("" : "+d"(v)); }
+// Asynchronous 8-byte copy global -> shared (LDGSTS).  The gathers of a chunk are issued back to back through these
+// and waited for ONCE: with plain loads ptxas places each dependent reciprocal right behind its load, and the warp
+// (in-order issue) then pays one round trip to L2 per field row — 17 of them per chunk (ncu, round 2).
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
 
-// Sort keys of the kPerThread cells base + threadIdx.x + j kThreads: the binary exponent of the norm bound
-// max_i a_i + sum_i eps_i a_i (R5), stiffest first, non-finite first of all; cells past the end last.
-// Species-major so that the loads of all the thread's cells for one species are in flight together.
-__device__ __forceinline__ void sort_keys(const UpdateArgs& G, int N, long long base, int count, unsigned* keys) {
-    const long long nc = G.ncells;
-    long long cell[kPerThread];
-    double irg[kPerThread], sb[kPerThread], amax[kPerThread];
+// One warp sorts the tile starting at cell `base` (count cells) into order[]: key = binary exponent of the norm bound
+// max_i a_i + sum_i eps_i a_i (R5), stiffest first, non-finite first of all, ties in cell order; entries
+// past `count` sort last.  keys: kTile words of scratch in the warp's own tile.  Species-major loads: all the lane's
+// cells for one species are in flight together.
+__device__ __noinline__ void sort_tile_warp(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                                            long long nc, int N, long long base, int count, unsigned* keys,
+                                            unsigned short* order, int lane) {
+    long long cell[kPerLane];
+    double irg[kPerLane], sb[kPerLane], amax[kPerLane];
 #pragma unroll
-    for (int j = 0; j < kPerThread; ++j) {
-        const int idx = threadIdx.x + j * kThreads;
+    for (int j = 0; j < kPerLane; ++j) {
+        const int idx = lane + j * 32;
         cell[j] = base + (idx < count ? idx : 0);
-        irg[j] = ldg_now(G.rho_g + cell[j]);
+        irg[j] = ldg_now(rho_g + cell[j]);
         sb[j] = 0.0;
         amax[j] = 0.0;
     }
 #pragma unroll
-    for (int j = 0; j < kPerThread; ++j) irg[j] = fast_rcp(irg[j]);
+    for (int j = 0; j < kPerLane; ++j) irg[j] = fast_rcp(irg[j]);
 #pragma unroll 2
     for (int i = 0; i < N; ++i) {
-        double ts[kPerThread], rd[kPerThread];
+        double ts[kPerLane], rd[kPerLane];
 #pragma unroll
-        for (int j = 0; j < kPerThread; ++j) {
-            ts[j] = ldg_now(G.t_s + (long long)i * nc + cell[j]);
-            rd[j] = ldg_now(G.rho_d + (long long)i * nc + cell[j]);
+        for (int j = 0; j < kPerLane; ++j) {
+            ts[j] = ldg_now(t_s + (long long)i * nc + cell[j]);
+            rd[j] = ldg_now(rho_d + (long long)i * nc + cell[j]);
         }
 #pragma unroll
-        for (int j = 0; j < kPerThread; ++j) {
-            const double a = G.dt * fast_rcp(ts[j]);
+        for (int j = 0; j < kPerLane; ++j) {
+            const double a = dt * fast_rcp(ts[j]);
             sb[j] = fma(rd[j] * irg[j], a, sb[j]);
             amax[j] = fmax(amax[j], a);
         }
     }
+    unsigned mine[kPerLane];
+    bool differs = false;
 #pragma unroll
-    for (int j = 0; j < kPerThread; ++j) {
-        const int idx = threadIdx.x + j * kThreads;
+    for (int j = 0; j < kPerLane; ++j) {
+        const int idx = lane + j * 32;
         const unsigned e = ((unsigned)__double2hiint(sb[j] + amax[j]) >> 20) & 0x7ffu;  // 0x7ff: Inf / NaN
         const unsigned key = (idx < count) ? 0x7ffu - e : 0xfffu;
-        keys[idx] = (key << 16) | (unsigned)idx;
+        mine[j] = (key << 16) | (unsigned)idx;
     }
-}
-
-__device__ __forceinline__ void sort_tile(unsigned* keys) {
-#pragma unroll 1
-    for (int k = 2; k <= kTile; k <<= 1) {
-#pragma unroll 1
-        for (int j = k >> 1; j > 0; j >>= 1) {
+    const unsigned k0 = __shfl_sync(kFullMask, mine[0], 0) >> 16;
 #pragma unroll
-            for (int t = threadIdx.x; t < kTile / 2; t += kThreads) {
-                const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
-                const int l = i | j;
-                const unsigned x = keys[i], y = keys[l];
-                const bool up = (i & k) == 0;
-                if ((x > y) == up) {
-                    keys[i] = y;
-                    keys[l] = x;
+    for (int j = 0; j < kPerLane; ++j) differs |= (lane + j * 32 < count) && ((mine[j] >> 16) != k0);
+    if (__any_sync(kFullMask, differs)) {  // (a tile whose cells all carry one key is already in order)
+#pragma unroll
+        for (int j = 0; j < kPerLane; ++j) keys[lane + j * 32] = mine[j];
+        __syncwarp();
+#pragma unroll 1
+        for (int k = 2; k <= kTile; k <<= 1) {
+#pragma unroll 1
+            for (int j = k >> 1; j > 0; j >>= 1) {
+#pragma unroll
+                for (int q = 0; q < kPerLane / 2; ++q) {
+                    const int t = lane + q * 32;
+                    const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                    const int l = i | j;
+                    const unsigned x = keys[i], y = keys[l];
+                    const bool up = (i & k) == 0;
+                    if ((x > y) == up) {
+                        keys[i] = y;
+                        keys[l] = x;
+                    }
                 }
+                __syncwarp();
             }
-            __syncthreads();
         }
+#pragma unroll
+        for (int j = 0; j < kPerLane; ++j) mine[j] = keys[lane + j * 32];
+        __syncwarp();
     }
+#pragma unroll
+    for (int j = 0; j < kPerLane; ++j) order[lane + j * 32] = (unsigned short)(mine[j] & 0xffffu);
 }
 
 __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* tiles = reinterpret_cast<double*>(smem_raw);
-    unsigned* keys = reinterpret_cast<unsigned*>(smem_raw);
-    unsigned short* order = reinterpret_cast<unsigned short*>(smem_raw + kMatBytes);
-    int* next_chunk = reinterpret_cast<int*>(smem_raw + kMatBytes + sizeof(unsigned short) * kTile);
+    Sched& sch = *reinterpret_cast<Sched*>(smem_raw + kTilesBytes);
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int r = lane >> 4, c = lane & 15;
     const long long nc = G.ncells;
     const int n = N + 1;
     const long long ntiles = (nc + kTile - 1) / kTile;
-    const typename Core::View V = Core::view(tiles + (size_t)warp * Core::CELL * CW, lane);
+    const int ktiles = (int)((ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x);  // tiles of this block
+    double* my_tile = tiles + (size_t)warp * Core::CELL * CW;
+    const typename Core::View V = Core::view(my_tile, lane);
 
-    for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const long long base = tile * kTile;
-        const int count = (nc - base < kTile) ? (int)(nc - base) : kTile;
-        // ---- 1. sort the tile by stiffness
-        sort_keys(G, N, base, count, keys);
-        if (threadIdx.x == 0) *next_chunk = 0;
-        __syncthreads();
-        // (a tile whose cells all carry one key is already in order)
-        const unsigned k0 = keys[0] >> 16;
-        int differs = 0;
-#pragma unroll
-        for (int j = 0; j < kPerThread; ++j) {
-            const int idx = threadIdx.x + j * kThreads;
-            differs |= (idx < count) && ((keys[idx] >> 16) != k0);
+    auto tile_base = [&](int k) { return ((long long)blockIdx.x + (long long)k * gridDim.x) * kTile; };
+    auto tile_count = [&](int k) {
+        const long long left = nc - tile_base(k);
+        return left < kTile ? (int)left : kTile;
+    };
+    // sorts tile k into its buffer and publishes it (called by ONE warp, whose own tile is free at that moment)
+    auto sort_and_publish = [&](int k) {
+        const int b = k % kBufs;
+        sort_tile_warp(G.rho_g, G.rho_d, G.t_s, G.dt, nc, N, tile_base(k), tile_count(k),
+                       reinterpret_cast<unsigned*>(my_tile), sch.order[b], lane);
+        __syncwarp();
+        __threadfence_block();
+        if (lane == 0) {
+            sch.next[b] = 0;
+            __threadfence_block();
+            *reinterpret_cast<volatile int*>(&sch.ready[b]) = k;
         }
-        if (__syncthreads_or(differs)) sort_tile(keys);
-        unsigned mine[kPerThread];
-#pragma unroll
-        for (int j = 0; j < kPerThread; ++j) mine[j] = keys[threadIdx.x + j * kThreads];
-        __syncthreads();  // keys (aliasing the warp tiles) are dead from here on
-#pragma unroll
-        for (int j = 0; j < kPerThread; ++j) order[threadIdx.x + j * kThreads] = (unsigned short)(mine[j] & 0xffffu);
-        __syncthreads();
-        const int nchunks = (count + CW - 1) / CW;
+        __syncwarp();
+    };
 
-        // ---- 2. chunks of 16 sorted cells
-        auto claim = [&]() {
+    if (threadIdx.x < kBufs) sch.ready[threadIdx.x] = -1;
+    __syncthreads();  // the only block-wide barrier
+    if (warp == 0) sort_and_publish(0);
+
+    // Claims the next chunk of this block: tile sequence number kc (advanced when a tile runs out), chunk index in the
+    // tile, and this lane's cell.  false when the block's tiles are exhausted.
+    int kc = 0;
+    auto claim = [&](long long& cell, bool& valid) {
+        for (;;) {
+            if (kc >= ktiles) return false;
+            const int b = kc % kBufs;
+            if (lane == 0)
+                while (*reinterpret_cast<volatile int*>(&sch.ready[b]) != kc) __nanosleep(64);
+            __syncwarp();
             int j = 0;
-            if (lane == 0) j = atomicAdd(next_chunk, 1);
-            return __shfl_sync(kFullMask, j, 0);
-        };
-        int jnext = claim();
-        while (jnext < nchunks) {
-            const int j = jnext;
-            jnext = claim();  // the chunk after this one (its fields are prefetched into L2 before this one's apply step)
-            const int pos = j * CW + c;
-            const bool valid = pos < count;
-            const long long cell = base + (valid ? (int)order[pos] : 0);
+            if (lane == 0) j = atomicAdd(&sch.next[b], 1);
+            j = __shfl_sync(kFullMask, j, 0);
+            const int count = tile_count(kc);
+            if (j * CW < count) {
+                const int pos = j * CW + c;
+                valid = pos < count;
+                cell = tile_base(kc) + (valid ? (int)*reinterpret_cast<volatile unsigned short*>(&sch.order[b][pos]) : 0);
+                // the first claimer of a tile sorts the next one before it starts on its chunk
+                if (j == 0 && kc + 1 < ktiles) sort_and_publish(kc + 1);
+                return true;
+            }
+            ++kc;
+        }
+    };
+
+    long long cell_n = 0;
+    bool valid_n = false;
+    bool have = claim(cell_n, valid_n);
+    while (have) {
+        const long long cell = cell_n;
+        const bool valid = valid_n;
+        {
+            // the chunk after this one is claimed now (its fields are prefetched into L2 before this one's apply step)
+            have = claim(cell_n, valid_n);
 
             // a1: eps_i (Eq. 14), a_i = dt / t_s,i (Eq. 15), symmetrising weights, for the species at my own positions
             double av[g], wv[g], iwv[g];
             double sbp = 0.0, amx = 0.0;
             {
-                double ts[g], rd[g];
-                const double rg = ldg_now(G.rho_g + cell);  // (an absent cell reads the tile's first cell)
-                static_for<0, g>([&](auto a) {  // all loads first: one round trip
+                // the fields travel into the (still unused) table: t_s -> col 2, rho_d -> col 3 of my own rows, rho_g ->
+                // my copy of the zz slot; a lane reads back only what it requested itself
+                static_for<0, g>([&](auto a) {
                     const int k = 2 * a + r;    // dust species at my own position a (an inert slot re-reads species 0)
                     const long long row = (long long)(k < N ? k : 0) * nc + cell;
-                    ts[a] = ldg_now(G.t_s + row);
-                    rd[a] = ldg_now(G.rho_d + row);
+                    cp_async8(&Core::at(V, 2 * a, 2), G.t_s + row);
+                    cp_async8(&Core::at(V, 2 * a, 3), G.rho_d + row);
                 });
+                cp_async8(&V.x[Core::ZZ * CW], G.rho_g + cell);  // (an absent cell reads the tile's first cell)
+                cp_async_wait_all();
+                double ts[g], rd[g];
+                const double rg = V.x[Core::ZZ * CW];
                 static_for<0, g>([&](auto a) {
-                    after_loads(ts[a]);
-                    after_loads(rd[a]);
+                    ts[a] = Core::at(V, 2 * a, 2);
+                    rd[a] = Core::at(V, 2 * a, 3);
                 });
                 const double irg = fast_rcp(rg);
                 static_for<0, g>([&](auto a) {
@@ -225,94 +282,91 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             }
             __syncwarp();
 
-            // a3: Taylor polynomial; a4: squarings (the last one is replaced by a second apply)
+            // a3: Taylor polynomial; a4: s squarings.  One loop: its first pass stores the polynomial, every later one
+            // squares first (one copy of the conservation / store code).
             typename Core::Acc A;
             Core::horner(V, m, -sb * sc, A);
-            const int nsq = max(s - Core::kDefer, 0);
-            const int napply = 1 << min(Core::kDefer, s);
-            Core::conserve_store(V, A, true, nsq == 0);
-            const int smax = __reduce_max_sync(kFullMask, nsq);
-            // Prefetches into L2, issued one phase ahead of their use — early enough to cover the HBM latency, late enough
-            // that the lines are still there (the tiles in flight on all SMs are larger than L2): this cell's momenta
-            // before the last squaring, the next chunk's fields before the apply step.
-            auto prefetch_momenta = [&]() {
-                if (valid) {
-                    static_for<0, 3>([&](auto cp) {
-                        static_for<0, g>([&](auto a) {
-                            const int k = 2 * a + r;
-                            if (k < N) prefetch_l2(G.p_in + ((long long)cp * n + 1 + k) * nc + cell);
-                        });
-                        if (r == 0) prefetch_l2(G.p_in + ((long long)cp * n) * nc + cell);
-                    });
+            const int smax = __reduce_max_sync(kFullMask, s);
+            for (int it = 0; it <= smax; ++it) {
+                if (it > 0) Core::square(V, c_tab, A);
+                if (it == smax) {
+                    // Prefetches into L2, one phase ahead of their use: this cell's momenta and the next chunk's fields.
+                    if (valid) {
+                        const double* pp = G.p_in + (long long)(1 + r) * nc + cell;
+#pragma unroll 1
+                        for (int cp = 0; cp < 3; ++cp) {
+                            prefetch_l2(G.p_in + (long long)cp * n * nc + cell);
+#pragma unroll 1
+                            for (int k = r; k < N; k += 2) prefetch_l2(pp + (long long)(k - r) * nc);
+                            pp += (long long)n * nc;
+                        }
+                    }
+                    if (have && valid_n) {
+                        prefetch_l2(G.rho_g + cell_n);
+#pragma unroll 1
+                        for (int k = r; k < N; k += 2) {
+                            prefetch_l2(G.t_s + (long long)k * nc + cell_n);
+                            prefetch_l2(G.rho_d + (long long)k * nc + cell_n);
+                        }
+                    }
                 }
-            };
-            if (smax == 0) prefetch_momenta();
-            for (int it = 0; it < smax; ++it) {
-                if (it == smax - 1) prefetch_momenta();
-                Core::square(V, c_tab, A);
-                Core::conserve_store(V, A, it < nsq, it == nsq - 1);
+                Core::conserve_store(V, A, it <= s, it == s);
             }
             if (valid && r == 0) {
                 if (G.s_out) G.s_out[cell] = s;
                 if (G.m_out) G.m_out[cell] = m;
             }
 
-            if (jnext < nchunks && jnext * CW + c < count) {
-                const long long cn = base + (int)order[jnext * CW + c];
-                if (r == 0) prefetch_l2(G.rho_g + cn);
-                static_for<0, g>([&](auto a) {
-                    const int k = 2 * a + r;
-                    if (k < N) {
-                        prefetch_l2(G.t_s + (long long)k * nc + cn);
-                        prefetch_l2(G.rho_d + (long long)k * nc + cn);
-                    }
-                });
-            }
-
-            // a5: p_out = p_in + W P W^-1 p_in (Eq. 18), applied 2^min(defer, s) times
+            // a5: p_out = p_in + W P W^-1 p_in (Eq. 18).  q = W^-1 p_in for all positions (own: loaded, other: from the
+            // partner lane), then one pass over the rows, each row's result going straight to global memory.
             {
-                double pu[3][g], p0[3], wu[g], iwu[g];
-                static_for<0, g>([&](auto a) {
-                    const int k = 2 * a + r;
-                    wu[a] = Core::at(V, 2 * a, Core::CWT);
-                    iwu[a] = Core::at(V, 2 * a, Core::CIW);
-                    static_for<0, 3>([&](auto cp) {
-                        pu[cp][a] = (valid && k < N) ? __ldg(G.p_in + ((long long)cp * n + 1 + k) * nc + cell) : 0.0;
-                    });
-                });
-                static_for<0, 3>([&](auto cp) { p0[cp] = valid ? __ldg(G.p_in + ((long long)cp * n) * nc + cell) : 0.0; });
-                const int amax_w = __reduce_max_sync(kFullMask, napply);
-                for (int rep = 0; rep < amax_w; ++rep) {
-                    const bool doit = rep < napply;
-                    double q[3][C];
+                double q[3][C], q0[3];
+                {
+                    const double* pp = G.p_in + (long long)(1 + r) * nc + cell;
                     static_for<0, 3>([&](auto cp) {
                         double qu[g], qo[g];
-                        static_for<0, g>([&](auto a) { qu[a] = pu[cp][a] * iwu[a]; });
+                        q0[cp] = valid ? G.p_in[(long long)cp * n * nc + cell] : 0.0;
+                        static_for<0, g>([&](auto a) {
+                            const int k = 2 * a + r;
+                            qu[a] = (valid && k < N) ? pp[(long long)(2 * a) * nc] : 0.0;
+                        });
+                        static_for<0, g>([&](auto a) { qu[a] *= Core::at(V, 2 * a, Core::CIW); });
                         static_for<0, g>([&](auto a) { qo[a] = __shfl_xor_sync(kFullMask, qu[a], 16); });
                         static_for<0, g>([&](auto a) {
                             q[cp][2 * a] = qu[a];
                             q[cp][2 * a + 1] = r ? qo[(a + 1) % g] : qo[a];  // my other position a is the partner's own
                         });
+                        pp += (long long)n * nc;
                     });
-                    double y0[3];
-                    Core::apply(V, q, p0, y0, [&](auto a, const double (&y)[3]) {
-                        static_for<0, 3>([&](auto cp) { pu[cp][a] = doit ? fma(wu[a], y[cp], pu[cp][a]) : pu[cp][a]; });
-                    });
-                    static_for<0, 3>([&](auto cp) { p0[cp] = doit ? p0[cp] + y0[cp] : p0[cp]; });
                 }
-                if (valid) {
-                    static_for<0, 3>([&](auto cp) {
-                        static_for<0, g>([&](auto a) {
-                            const int k = 2 * a + r;
-                            if (k < N) G.p_out[((long long)cp * n + 1 + k) * nc + cell] = pu[cp][a];
+                const double* pin = G.p_in + (long long)(1 + r) * nc + cell;
+                double* pout = G.p_out + (long long)(1 + r) * nc + cell;
+                const long long comp_stride = (long long)n * nc;
+#pragma unroll 1
+                for (int a = 0; a < g; ++a) {  // my own dust rows: species k = 2a + r
+                    double y[3];
+                    Core::apply_row(V, c_tab.ap[a], q, q0, y);
+                    const double w = V.x[((2 * a) * Core::ROW + Core::CWT) * CW];
+                    if (valid && 2 * a + r < N) {
+                        static_for<0, 3>([&](auto cp) {
+                            pout[cp * comp_stride] = fma(w, y[cp], pin[cp * comp_stride]);
                         });
-                        if (r == 0) G.p_out[((long long)cp * n) * nc + cell] = p0[cp];
-                    });
+                    }
+                    pin += 2 * nc;
+                    pout += 2 * nc;
+                }
+                {  // the gas row (both lanes compute it, role 0 stores it)
+                    double y[3];
+                    Core::apply_row(V, c_tab.ap[g], q, q0, y);
+                    if (valid && r == 0) {
+                        static_for<0, 3>([&](auto cp) {
+                            G.p_out[cp * comp_stride + cell] = G.p_in[cp * comp_stride + cell] + y[cp];
+                        });
+                    }
                 }
             }
             __syncwarp();  // both lanes of a pair are done with the tile before the next chunk's scratch overwrites it
         }
-        __syncthreads();  // all chunks of this tile are done: the tiles may be reused as the sort buffer
     }
 }
 
