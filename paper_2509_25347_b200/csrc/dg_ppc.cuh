@@ -189,30 +189,44 @@ struct Ppc {
     // step is P = X - I) and the copies the rotated addressing needs.  `active` = this cell still takes part.
     __device__ __forceinline__ static void conserve_store(const View& V, const Acc& A, bool active, bool fin) {
         const int r = V.r;
+        // (three short independent chains per own column — own pairs above, own pairs below, mixed pairs — so that the
+        // fp64 pipe's 8-cycle dependent latency is hidden inside the lane)
         double cu[g], co[g], cz = 0.0;
         double wu[g], wo[g];
         static_for<0, g>([&](auto a) {
             wu[a] = at(V, 2 * a, CWT);
             wo[a] = at(V, 2 * a + 1, CWT);
-            cu[a] = 0.0;
-            co[a] = 0.0;
         });
-        static_for<0, g>([&](auto a) {
-            static_for<a + 1, g>([&](auto b) {
-                const double v = A.T[tix(a, b)];
-                cu[a] = fma(wu[b], v, cu[a]);
-                cu[b] = fma(wu[a], v, cu[b]);
+        {
+            double ca[g], cb[g], cm[g];
+            static_for<0, g>([&](auto a) {
+                ca[a] = A.Z[a];  // the gas row's entry: w_z = 1
+                cb[a] = 0.0;
+                cm[a] = 0.0;
+                co[a] = 0.0;
             });
-            static_for<0, D>([&](auto dd) {
-                constexpr int b = (a + dd) % g;
-                double v = A.M[a][dd];
-                if constexpr (kDupClass && dd == D - 1) v = r ? 0.0 : v;  // counted by role 0 only
-                cu[a] = fma(wo[b], v, cu[a]);
-                co[b] = fma(wu[a], v, co[b]);
+            static_for<0, g>([&](auto a) {
+                static_for<a + 1, g>([&](auto b) {
+                    const double v = A.T[tix(a, b)];
+                    ca[a] = fma(wu[b], v, ca[a]);
+                    cb[b] = fma(wu[a], v, cb[b]);
+                });
+                static_for<0, D>([&](auto dd) {
+                    constexpr int b = (a + dd) % g;
+                    double v = A.M[a][dd];
+                    if constexpr (kDupClass && dd == D - 1) v = r ? 0.0 : v;  // counted by role 0 only
+                    cm[a] = fma(wo[b], v, cm[a]);
+                    co[b] = fma(wu[a], v, co[b]);
+                });
             });
-            cu[a] += A.Z[a];
-            cz = fma(wu[a], A.Z[a], cz);
-        });
+            double cza = 0.0, czb = 0.0;
+            static_for<0, g>([&](auto a) {
+                cu[a] = (ca[a] + cb[a]) + cm[a];
+                if constexpr (a % 2 == 0) cza = fma(wu[a], A.Z[a], cza);
+                else czb = fma(wu[a], A.Z[a], czb);
+            });
+            cz = cza + czb;
+        }
         // partner's sums for MY own columns: its other-position b is my own position a = b + 1 - r_partner
         double dgl[g];
         static_for<0, g>([&](auto b) { co[b] = __shfl_xor_sync(0xffffffffu, co[b], 16); });
@@ -301,9 +315,20 @@ struct Ppc {
                     A.M[a][dd] = fma(-alo[b], A.M[a][dd], vu[a]);
                 });
             });
-            double t00 = b2u[0] * vu[0];
-            static_for<1, g>([&](auto a) { t00 = fma(b2u[a], vu[a], t00); });
-            static_for<0, g>([&](auto a) { t00 = fma(b2o[a], vo[a], t00); });
+            double t00;
+            {  // sum_l beta_l^2 v_l in four independent chains
+                double ta = b2u[0] * vu[0], tb = b2o[0] * vo[0], tc = 0.0, td = 0.0;
+                static_for<1, g>([&](auto a) {
+                    if constexpr (a % 2 == 1) {
+                        tc = fma(b2u[a], vu[a], tc);
+                        td = fma(b2o[a], vo[a], td);
+                    } else {
+                        ta = fma(b2u[a], vu[a], ta);
+                        tb = fma(b2o[a], vo[a], tb);
+                    }
+                });
+                t00 = (ta + tb) + (tc + td);
+            }
             const double x00 = kap + q00;
             static_for<0, g>([&](auto a) {
                 vu[a] = fma(-alu[a], vu[a], x00);

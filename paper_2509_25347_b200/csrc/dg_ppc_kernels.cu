@@ -290,7 +290,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             for (int it = 0; it <= smax; ++it) {
                 if (it > 0) Core::square(V, c_tab, A);
                 if (it == smax) {
-                    // Prefetches into L2, one phase ahead of their use: this cell's momenta and the next chunk's fields.
+                    // This cell's momenta (never touched so far) start their way from HBM to L2 one squaring ahead of the
+                    // apply step.  (The fields of the next chunk need no prefetch: the warp that sorted the tile read them.)
                     if (valid) {
                         const double* pp = G.p_in + (long long)(1 + r) * nc + cell;
 #pragma unroll 1
@@ -299,14 +300,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
 #pragma unroll 1
                             for (int k = r; k < N; k += 2) prefetch_l2(pp + (long long)(k - r) * nc);
                             pp += (long long)n * nc;
-                        }
-                    }
-                    if (have && valid_n) {
-                        prefetch_l2(G.rho_g + cell_n);
-#pragma unroll 1
-                        for (int k = r; k < N; k += 2) {
-                            prefetch_l2(G.t_s + (long long)k * nc + cell_n);
-                            prefetch_l2(G.rho_d + (long long)k * nc + cell_n);
                         }
                     }
                 }
@@ -342,17 +335,28 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                 const double* pin = G.p_in + (long long)(1 + r) * nc + cell;
                 double* pout = G.p_out + (long long)(1 + r) * nc + cell;
                 const long long comp_stride = (long long)n * nc;
+                // my own dust rows, species k = 2a + r; the row's p_in values are requested two rows ahead (they were read
+                // once for q, but a gather of 27 rows does not survive in what is left of L1 beside the 217 KB of tiles)
+                auto load_p = [&](int a, double (&pv)[3]) {
+                    const bool live = valid && 2 * a + r < N;
+                    static_for<0, 3>([&](auto cp) { pv[cp] = live ? pin[(long long)(2 * a) * nc + cp * comp_stride] : 0.0; });
+                };
+                double pa[3], pb[3];
+                load_p(0, pa);
+                load_p(g > 1 ? 1 : 0, pb);
 #pragma unroll 1
-                for (int a = 0; a < g; ++a) {  // my own dust rows: species k = 2a + r
-                    double y[3];
+                for (int a = 0; a < g; ++a) {
+                    double pc[3], y[3];
+                    static_for<0, 3>([&](auto cp) {
+                        pc[cp] = pa[cp];
+                        pa[cp] = pb[cp];
+                    });
+                    load_p(a + 2 < g ? a + 2 : g - 1, pb);
                     Core::apply_row(V, c_tab.ap[a], q, q0, y);
                     const double w = V.x[((2 * a) * Core::ROW + Core::CWT) * CW];
                     if (valid && 2 * a + r < N) {
-                        static_for<0, 3>([&](auto cp) {
-                            pout[cp * comp_stride] = fma(w, y[cp], pin[cp * comp_stride]);
-                        });
+                        static_for<0, 3>([&](auto cp) { pout[cp * comp_stride] = fma(w, y[cp], pc[cp]); });
                     }
-                    pin += 2 * nc;
                     pout += 2 * nc;
                 }
                 {  // the gas row (both lanes compute it, role 0 stores it)
