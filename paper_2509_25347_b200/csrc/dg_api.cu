@@ -33,11 +33,15 @@ static const PpcLaunchers* const kPpcTable[DG_NMAX + 1] = {
     &ppc_launchers_NP14, &ppc_launchers_NP14, &ppc_launchers_NP16, &ppc_launchers_NP16};
 
 // The mapping dg_drag_update uses for each N, chosen from measurements on B200: the thread-per-cell
-// kernel keeps the packed symmetric matrices of one cell in registers up to N = 9 and spills mildly up to N = 13, where
-// it still wins (2^21 stiff cells: 8.1 vs 11.3 ms at N = 13, 21.5 vs 11.4 ms at N = 14); from N = 14 its spills take
-// over and the warp-per-cell DMMA kernel wins.
-constexpr int kFirstWpcN = 14;
-static inline int default_variant(int N) { return N >= kFirstWpcN ? DG_VARIANT_WPC : DG_VARIANT_TPC; }
+// kernel keeps the packed symmetric matrices of one cell in registers up to N = 9 and spills mildly up to N = 12, where
+// it still wins; from N = 13 its spills take over and the pair-per-cell kernel (two lanes per cell, the iterate in a
+// shared-memory tile) wins (2^22 stiff cells, ms: N = 12: 7.0 thread / 7.9 pair; N = 13: 16.2 / 11.2; N = 16: - / 14.8,
+// warp-per-cell DMMA 23.1).
+constexpr int kFirstPpcN = 13;
+static inline int default_variant(int N) { return N >= kFirstPpcN ? DG_VARIANT_PPC : DG_VARIANT_TPC; }
+// The staged dg_expm_scale_square has no pair-per-cell form (it writes dense matrices to HBM: a test path); it keeps the
+// warp-per-cell DMMA kernel from N = 14 and the thread-per-cell one below.
+static inline int expm_variant(int N) { return N >= 14 ? DG_VARIANT_WPC : DG_VARIANT_TPC; }
 
 static thread_local char g_cuda_err[256] = "";
 
@@ -105,7 +109,7 @@ dg_status dg_expm_scale_square(const double* A, int N, long long ncells, double*
     DG_CHECK_OPT_PTR(s_out);
     ExpmArgs a{A, ncells, E, s_out};
     cudaStream_t cs = static_cast<cudaStream_t>(stream);
-    return cuda_status(default_variant(N) == DG_VARIANT_WPC ? kWpcTable[N]->expm(a, cs) : kTable[N]->expm(a, cs));
+    return cuda_status(expm_variant(N) == DG_VARIANT_WPC ? kWpcTable[N]->expm(a, cs) : kTable[N]->expm(a, cs));
 }
 
 dg_status dg_drag_apply(const double* E, const double* p_in, int N, long long ncells, double* p_out, void* stream) {
@@ -194,7 +198,7 @@ int dg_launches_per_update(int N, long long ncells) {
 
 const char* dg_variant_name(int N) {
     if (N < 1 || N > DG_NMAX) return "";
-    return default_variant(N) == DG_VARIANT_WPC ? kWpcTable[N]->variant : kTable[N]->variant;
+    return default_variant(N) == DG_VARIANT_PPC ? kPpcTable[N]->variant : kTable[N]->variant;
 }
 
 const char* dg_status_string(dg_status st) {

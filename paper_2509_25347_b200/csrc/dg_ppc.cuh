@@ -186,17 +186,52 @@ struct Ppc {
     // The diagonal from conservation of total momentum:  d_j = -(sum_{i != j} w_i O_ij) / w_j  (w_z = 1).  Every lane
     // sums its own entries into the columns they touch; the partner's share of a lane's own columns comes by shuffle.
     // Writes the off-diagonals, the diagonal (X_jj = 1 + d_j, or d_j itself when `fin`: the matrix handed to the apply
-    // step is P = X - I) and the copies the rotated addressing needs.  `active` = this cell still takes part.
-    __device__ __forceinline__ static void conserve_store(const View& V, const Acc& A, bool active, bool fin) {
+    // step is P = X - I) and the copies the rotated addressing needs.  `fin` is warp-uniform.
+    __device__ __forceinline__ static void conserve_store(const View& V, const Acc& A, bool fin) {
+        constexpr bool active = true;  // every lane of the warp runs the same number of squarings (see the kernel)
         const int r = V.r;
-        // (three short independent chains per own column — own pairs above, own pairs below, mixed pairs — so that the
-        // fp64 pipe's 8-cycle dependent latency is hidden inside the lane)
-        double cu[g], co[g], cz = 0.0;
+        const bool r0 = (r == 0);
         double wu[g], wo[g];
         static_for<0, g>([&](auto a) {
             wu[a] = at(V, 2 * a, CWT);
             wo[a] = at(V, 2 * a + 1, CWT);
         });
+        __syncwarp();  // every lane has finished reading the old matrix (or the Horner scratch)
+        // The off-diagonal stores come FIRST in program order and are unconditional (but for the role-0 copies), so that
+        // the scheduler can interleave them with the sums below: 96 back-to-back STS.64 cost a lane ~6 issue cycles
+        // each with nothing else to do (9 % of the kernel, ncu round 2); the sums keep the fp64 pipe busy meanwhile.
+        auto st = [&](int idx, double v, bool pred) {
+            if (pred) V.x[idx * CW] = v;
+        };
+        static_for<0, g>([&](auto a) {
+            static_for<a + 1, g>([&](auto b) {
+                constexpr int s1 = slot(2 * a, 2 * b), s2 = slot2(2 * a, 2 * b);
+                const double v = A.T[tix(a, b)];
+                st(s1, v, active);
+                if constexpr (s2 >= 0) st(s2, v, active);
+                if constexpr (s1 / ROW == 0) st(s1 + C * ROW, v, active && r0);  // row C = copy of row 0 (role 0's)
+            });
+            static_for<0, D>([&](auto dd) {
+                constexpr int q = opos((a + dd) % g);
+                constexpr int s1 = slot(2 * a, q), s2 = slot2(2 * a, q);
+                const double v = A.M[a][dd];
+                if constexpr (kDupClass && dd == D - 1) {  // antipodal class: role 0 stores both slots
+                    st(s1, v, active && r0);
+                    st(s2, v, active && r0);
+                    if constexpr (s1 / ROW == 0) st(s1 + C * ROW, v, active && r0);
+                    if constexpr (s2 / ROW == 0) st(s2 + C * ROW, v, active && r0);
+                } else {
+                    st(s1, v, active);
+                    if constexpr (s2 >= 0) st(s2, v, active);
+                    if constexpr (s1 / ROW == 0) st(s1 + C * ROW, v, active && r0);
+                }
+            });
+            st((2 * a) * ROW + CZ, A.Z[a], active);
+            if constexpr (a == 0) st(C * ROW + CZ, A.Z[a], active && r0);
+        });
+        // (three short independent chains per own column — own pairs above, own pairs below, mixed pairs — so that the
+        // fp64 pipe's 8-cycle dependent latency is hidden inside the lane)
+        double cu[g], co[g], cz = 0.0;
         {
             double ca[g], cb[g], cm[g];
             static_for<0, g>([&](auto a) {
@@ -228,59 +263,19 @@ struct Ppc {
             cz = cza + czb;
         }
         // partner's sums for MY own columns: its other-position b is my own position a = b + 1 - r_partner
-        double dgl[g];
         static_for<0, g>([&](auto b) { co[b] = __shfl_xor_sync(0xffffffffu, co[b], 16); });
         static_for<0, g>([&](auto a) {
             const double pv = r ? co[a] : co[(a + g - 1) % g];
             const double d = -(cu[a] + pv) * at(V, 2 * a, CIW);
-            dgl[a] = fin ? d : 1.0 + d;
+            const double dgl = fin ? d : 1.0 + d;
+            st((2 * a) * ROW, dgl, active);
+            if constexpr (a == 0) st(C * ROW, dgl, active && r0);
         });
         {
             const double other = __shfl_xor_sync(0xffffffffu, cz, 16);
             const double lo = r ? other : cz, hi = r ? cz : other;  // same order in both lanes
             cz = -(lo + hi);
-            cz = fin ? cz : 1.0 + cz;
-        }
-        __syncwarp();  // every lane has finished reading the old matrix (or the Horner scratch)
-        if (active) {
-            const bool r0 = (r == 0);
-            static_for<0, g>([&](auto a) {
-                static_for<a + 1, g>([&](auto b) {
-                    constexpr int s1 = slot(2 * a, 2 * b), s2 = slot2(2 * a, 2 * b);
-                    const double v = A.T[tix(a, b)];
-                    V.x[s1 * CW] = v;
-                    if constexpr (s2 >= 0) V.x[s2 * CW] = v;
-                    if constexpr (s1 / ROW == 0)
-                        if (r0) V.x[(s1 + C * ROW) * CW] = v;  // row C = copy of row 0 (row 0 belongs to role 0)
-                });
-                static_for<0, D>([&](auto dd) {
-                    constexpr int q = opos((a + dd) % g);
-                    constexpr int s1 = slot(2 * a, q), s2 = slot2(2 * a, q);
-                    const double v = A.M[a][dd];
-                    if constexpr (kDupClass && dd == D - 1) {  // antipodal class: role 0 stores both slots
-                        if (r0) {
-                            V.x[s1 * CW] = v;
-                            V.x[s2 * CW] = v;
-                            if constexpr (s1 / ROW == 0) V.x[(s1 + C * ROW) * CW] = v;
-                            if constexpr (s2 / ROW == 0) V.x[(s2 + C * ROW) * CW] = v;
-                        }
-                    } else {
-                        V.x[s1 * CW] = v;
-                        if constexpr (s2 >= 0) V.x[s2 * CW] = v;
-                        if constexpr (s1 / ROW == 0)
-                            if (r0) V.x[(s1 + C * ROW) * CW] = v;
-                    }
-                });
-                at(V, 2 * a, CZ) = A.Z[a];
-                at(V, 2 * a, 0) = dgl[a];
-                if constexpr (a == 0) {
-                    if (r0) {
-                        at(V, C, CZ) = A.Z[a];
-                        at(V, C, 0) = dgl[a];
-                    }
-                }
-            });
-            V.x[ZZ * CW] = cz;  // each role its own copy
+            st(ZZ, fin ? cz : 1.0 + cz, active);  // each role its own copy
         }
         __syncwarp();
     }

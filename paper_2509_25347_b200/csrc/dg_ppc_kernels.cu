@@ -262,6 +262,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             int m, s;
             choose_m_s_warp(norm, Core::hcost(), m, s);
             m = __reduce_max_sync(kFullMask, m);  // already uniform; REDUX puts it in a uniform register
+            // Every cell of the chunk runs the LARGEST s among its 16 cells: any s' >= s satisfies Theorem 1's premise
+            // a fortiori, the lanes would idle through those squarings otherwise, and with one s per
+            // warp no store is predicated.  After the sort the chunk's cells differ by at most one in s anyway.
+            s = __reduce_max_sync(kFullMask, s);
             const double sc = pow2neg(s);
             {
                 static_for<0, g>([&](auto a) {
@@ -286,7 +290,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             // squares first (one copy of the conservation / store code).
             typename Core::Acc A;
             Core::horner(V, m, -sb * sc, A);
-            const int smax = __reduce_max_sync(kFullMask, s);
+            const int smax = s;
             for (int it = 0; it <= smax; ++it) {
                 if (it > 0) Core::square(V, c_tab, A);
                 if (it == smax) {
@@ -303,7 +307,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                         }
                     }
                 }
-                Core::conserve_store(V, A, it <= s, it == s);
+                Core::conserve_store(V, A, it == smax);
             }
             if (valid && r == 0) {
                 if (G.s_out) G.s_out[cell] = s;
