@@ -73,7 +73,7 @@ struct Ppc {
     __host__ __device__ static constexpr int opos(int b) { return md(2 * b + 1); }  // other position b, role 0
 
     // fp64-pipe instructions of one Horner step and one squaring per lane: prices the polynomial in choose_m_s
-    static constexpr int kHornerOps = NT + g * D + 4 * g + 3;
+    static constexpr int kHornerOps = NT + g * D + 2 * g + 5;
     static constexpr int kSquareOps = n * (NT + g * D + g) + 2 * (NT + g * D + g) + 3 * g;
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
@@ -94,10 +94,22 @@ struct Ppc {
     // ap[a][j]: the operands of row a of the apply step, a = 0..g-1 the lane's own positions and a = g the gas row:
     // ap[a][j] = X[own a][position j], j = 0..C-1 (j = 2a: the diagonal), ap[a][C] = X[own a][z]; for the gas row
     // ap[g][j] = X[z][position j], ap[g][C] = X[z][z].
-    struct Tab {
-        int sq[C + 1][C + 1];
-        int ap[g + 1][C + 1];
+    static constexpr int RW = ((C + 1 + 3) / 4) * 4;  // table rows padded to 16 bytes: four offsets per constant load
+    struct alignas(16) Tab {
+        int sq[C + 1][RW];
+        int ap[g + 1][RW];
     };
+    // the C + 1 offsets of one table row, fetched four at a time (LDCU.128)
+    __device__ __forceinline__ static void row_offsets(const int* row, int (&off)[RW]) {
+        const int4* r4 = reinterpret_cast<const int4*>(row);
+        static_for<0, RW / 4>([&](auto i) {
+            const int4 v = r4[i];
+            off[4 * i] = v.x;
+            off[4 * i + 1] = v.y;
+            off[4 * i + 2] = v.z;
+            off[4 * i + 3] = v.w;
+        });
+    }
     __host__ __device__ static constexpr Tab make_tab() {
         Tab t{};
         for (int l = 0; l < C; ++l) {
@@ -144,7 +156,9 @@ struct Ppc {
     struct RowOps {  // the n operands of one row l
         double u[g], o[g], z;
     };
-    __device__ __forceinline__ static void load_row(const View& V, const int* off, RowOps& R) {
+    __device__ __forceinline__ static void load_row(const View& V, const int* row, RowOps& R) {
+        int off[RW];
+        row_offsets(row, off);
         static_for<0, g>([&](auto a) {
             R.u[a] = lds(V.x, off[2 * a]);
             R.o[a] = lds(V.x, off[2 * a + 1]);
@@ -283,26 +297,33 @@ struct Ppc {
     // ---- Taylor polynomial T_m(S / 2^s) - I  (Eq. 19), factored Horner recurrence of dg_tpc.cuh ----------------------
     // Q_j = (m!/j!) P_j,  Q_0k = beta_k v_k,  Q_ik = beta_i beta_k U_ik:
     //     U_ik <- v_k - alpha_i U_ik,   v_k <- (kappa_j + Q_00) - alpha_k v_k,   Q_00 <- b00 (kappa_j + Q_00) + sum_l beta_l^2 v_l
-    // (right-hand sides: old values).  The lane owns U for its pairs (T: own a, own b; M: own a, other b) and carries
-    // v at all C positions (its own and the other role's: 2 g FMAs more per step, no cross-lane traffic in the loop).
+    // (right-hand sides: old values).  The lane owns U for its pairs (T: own a, own b; M: own a, other b) and v at its
+    // own positions; the only cross-lane traffic of a step is the partner's half of the sum (one 64-bit shuffle).
     // For an M pair the recurrence is used in its mirrored form U <- v_own - alpha_other U (B Q is symmetric).
     // alpha, beta (already scaled by 2^-s) are read from the Horner scratch in shared memory.  m is warp-uniform.
     __device__ __forceinline__ static void horner(const View& V, int m, double b00, Acc& A) {
-        double alu[g], alo[g], b2u[g], b2o[g], vu[g], vo[g];
+        double alu[g], alo[g], b2u[g], vu[g];
         static_for<0, g>([&](auto a) {
             alu[a] = at(V, 2 * a, CAL);
             alo[a] = at(V, 2 * a + 1, CAL);
-            const double bu = at(V, 2 * a, CBE), bo = at(V, 2 * a + 1, CBE);
+            const double bu = at(V, 2 * a, CBE);
             b2u[a] = bu * bu;
-            b2o[a] = bo * bo;
             vu[a] = 1.0;
-            vo[a] = 1.0;
             static_for<0, D>([&](auto dd) { A.M[a][dd] = 0.0; });
         });
         static_for<0, (NT > 0 ? NT : 1)>([&](auto K) { A.T[K] = 0.0; });
         double q00 = b00, kap = 1.0;
         for (int j = m - 1; j >= 1; --j) {
             kap *= c_dbl[j + 1];
+            // sum_l beta_l^2 v_l: my own positions here (two chains), the partner's half by shuffle; the U updates below
+            // do not depend on it and cover the shuffle's latency
+            double ta = b2u[0] * vu[0], tb = 0.0;
+            static_for<1, g>([&](auto a) {
+                if constexpr (a % 2 == 1) tb = fma(b2u[a], vu[a], tb);
+                else ta = fma(b2u[a], vu[a], ta);
+            });
+            const double tmine = ta + tb;
+            const double tother = __shfl_xor_sync(0xffffffffu, tmine, 16);
             static_for<0, g>([&](auto a) {
                 static_for<a + 1, g>([&](auto b) { A.T[tix(a, b)] = fma(-alu[a], A.T[tix(a, b)], vu[b]); });
                 static_for<0, D>([&](auto dd) {
@@ -310,25 +331,9 @@ struct Ppc {
                     A.M[a][dd] = fma(-alo[b], A.M[a][dd], vu[a]);
                 });
             });
-            double t00;
-            {  // sum_l beta_l^2 v_l in four independent chains
-                double ta = b2u[0] * vu[0], tb = b2o[0] * vo[0], tc = 0.0, td = 0.0;
-                static_for<1, g>([&](auto a) {
-                    if constexpr (a % 2 == 1) {
-                        tc = fma(b2u[a], vu[a], tc);
-                        td = fma(b2o[a], vo[a], td);
-                    } else {
-                        ta = fma(b2u[a], vu[a], ta);
-                        tb = fma(b2o[a], vo[a], tb);
-                    }
-                });
-                t00 = (ta + tb) + (tc + td);
-            }
+            const double t00 = (V.r ? tother : tmine) + (V.r ? tmine : tother);  // same order in both lanes
             const double x00 = kap + q00;
-            static_for<0, g>([&](auto a) {
-                vu[a] = fma(-alu[a], vu[a], x00);
-                vo[a] = fma(-alo[a], vo[a], x00);
-            });
+            static_for<0, g>([&](auto a) { vu[a] = fma(-alu[a], vu[a], x00); });
             q00 = fma(b00, x00, t00);
         }
         // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!; off-diagonals are >= 0 in exact arithmetic
@@ -350,8 +355,10 @@ struct Ppc {
     // q[comp][j] (j = 0..C-1 in role-rotated order: index j <-> position j + r) and q0[comp] are the three W^-1 p_in
     // vectors; `off` = tab.ap[row].  Returns y[comp] = P[row][z] q0 + sum_j P[row][j] q_j.  Two partial sums per
     // component (six independent FMA chains).  The caller loops over the rows: the code is the same for every row.
-    __device__ __forceinline__ static void apply_row(const View& V, const int* off, const double (&q)[3][C],
+    __device__ __forceinline__ static void apply_row(const View& V, const int* row, const double (&q)[3][C],
                                                      const double (&q0)[3], double (&y)[3]) {
+        int off[RW];
+        row_offsets(row, off);
         double e[C + 1];
         static_for<0, C + 1>([&](auto j) { e[j] = lds(V.x, off[j]); });
         double ya[3], yb[3];

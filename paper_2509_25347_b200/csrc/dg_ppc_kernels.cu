@@ -297,13 +297,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                     // This cell's momenta (never touched so far) start their way from HBM to L2 one squaring ahead of the
                     // apply step.  (The fields of the next chunk need no prefetch: the warp that sorted the tile read them.)
                     if (valid) {
-                        const double* pp = G.p_in + (long long)(1 + r) * nc + cell;
+                        const long long step = 2 * nc;
+                        const double* pg = G.p_in + cell;
 #pragma unroll 1
                         for (int cp = 0; cp < 3; ++cp) {
-                            prefetch_l2(G.p_in + (long long)cp * n * nc + cell);
-#pragma unroll 1
-                            for (int k = r; k < N; k += 2) prefetch_l2(pp + (long long)(k - r) * nc);
-                            pp += (long long)n * nc;
+                            if (r == 0) prefetch_l2(pg);
+                            const double* pd = pg + (long long)(1 + r) * nc;
+#pragma unroll 4
+                            for (int k = r; k < N; k += 2) {
+                                prefetch_l2(pd);
+                                pd += step;
+                            }
+                            pg += (long long)n * nc;
                         }
                     }
                 }
