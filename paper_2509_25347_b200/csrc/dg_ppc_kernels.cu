@@ -11,9 +11,10 @@
 //     deterministic, no block barrier;
 //   * all warps claim chunks of 16 sorted cells from the tile's counter; the warp that claims the FIRST chunk of tile k
 //     sorts tile k + 1 before it starts on its chunk, so the next tile is ready long before this one runs out
-//     (three order buffers: the one being overwritten belongs to tile k - 2).  No warp ever waits for another one
-//     except at the very start.
-// Loads and stores of the fields are gathers inside a tile.  A tile is small (256 cells, 172 KB of fields) so that the
+//     (three order buffers: the one being overwritten belongs to tile k - 2, and a warp that comes back to a buffer
+//     after it has moved on to a later tile sees that from the sequence number in the buffer's state word).  No warp
+//     waits for another one except at the very start.
+// Loads and stores of the fields are gathers inside a tile.  A tile is small (128 cells, 86 KB of fields) so that the
 // tiles in flight on all SMs stay L2-resident: with 2048-cell tiles they did not (5.6 KB of DRAM reads per cell for
 // 0.94 KB needed, ncu round 2), because a 32-byte sector fetched for one cell was evicted before its three neighbours
 // were processed.
@@ -32,16 +33,19 @@ using Core = Ppc<NP>;
 constexpr int C = Core::C, g = Core::g, CW = Core::CW;
 constexpr int kWarps = 8;
 constexpr int kThreads = 32 * kWarps;
-constexpr int kTile = 256;
+constexpr int kTile = 128;
 constexpr int kPerLane = kTile / 32;
 constexpr int kBufs = 3;
 constexpr unsigned kFullMask = 0xffffffffu;
 
 struct Sched {  // block-wide scheduling state
     unsigned short order[kBufs][kTile];  // sorted cell offsets of the tiles in flight
-    int next[kBufs];                     // chunk claim counter
-    int ready[kBufs];                    // sequence number of the tile whose order is in the buffer (-1: none)
+    // per buffer: ((sequence number of the tile whose order is in the buffer) + 1) << 8 | chunks claimed so far; 0 = none.
+    // One word, so that publishing a tile, claiming a chunk (compare-and-swap) and noticing that the buffer has moved on
+    // to a later tile are each a single atomic access.
+    unsigned state[kBufs];
 };
+static_assert(kTile / 16 < 256, "the chunk counter lives in the low byte of Sched::state");
 constexpr size_t kTilesBytes = Core::kWarpBytes * kWarps;
 static_assert(Core::kWarpBytes >= sizeof(unsigned) * kTile, "a warp sorts a tile inside its own shared-memory tile");
 constexpr size_t kSmemBytes = kTilesBytes + sizeof(Sched);
@@ -169,15 +173,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                        reinterpret_cast<unsigned*>(my_tile), sch.order[b], lane);
         __syncwarp();
         __threadfence_block();
-        if (lane == 0) {
-            sch.next[b] = 0;
-            __threadfence_block();
-            *reinterpret_cast<volatile int*>(&sch.ready[b]) = k;
-        }
+        if (lane == 0) *reinterpret_cast<volatile unsigned*>(&sch.state[b]) = (unsigned)(k + 1) << 8;
         __syncwarp();
     };
 
-    if (threadIdx.x < kBufs) sch.ready[threadIdx.x] = -1;
+    if (threadIdx.x < kBufs) sch.state[threadIdx.x] = 0;
     __syncthreads();  // the only block-wide barrier
     if (warp == 0) sort_and_publish(0);
 
@@ -188,16 +188,30 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
         for (;;) {
             if (kc >= ktiles) return false;
             const int b = kc % kBufs;
-            if (lane == 0)
-                while (*reinterpret_cast<volatile int*>(&sch.ready[b]) != kc) __nanosleep(64);
-            __syncwarp();
-            int j = 0;
-            if (lane == 0) j = atomicAdd(&sch.next[b], 1);
-            j = __shfl_sync(kFullMask, j, 0);
             const int count = tile_count(kc);
-            if (j * CW < count) {
+            const int nchunks = (count + CW - 1) / CW;
+            int j = 0;
+            if (lane == 0) {
+                volatile unsigned* st = &sch.state[b];
+                for (;;) {
+                    const unsigned v = *st;
+                    const int seq = (int)(v >> 8) - 1;
+                    if (seq < kc) {  // not sorted yet (only at the very start, or behind a slow sorter)
+                        __nanosleep(64);
+                        continue;
+                    }
+                    j = (int)(v & 0xffu);
+                    if (seq > kc) j = nchunks;  // the buffer already holds a later tile: this one ran out long ago
+                    if (j >= nchunks) break;
+                    if (atomicCAS(&sch.state[b], v, v + 1) == v) break;
+                }
+            }
+            j = __shfl_sync(kFullMask, j, 0);
+            if (j < nchunks) {
                 const int pos = j * CW + c;
                 valid = pos < count;
+                // (the buffer cannot be recycled between the claim and this read: that takes two more tiles' worth of
+                // claims by the other warps and a sort, which starts with a round trip to HBM)
                 cell = tile_base(kc) + (valid ? (int)*reinterpret_cast<volatile unsigned short*>(&sch.order[b][pos]) : 0);
                 // the first claimer of a tile sorts the next one before it starts on its chunk
                 if (j == 0 && kc + 1 < ktiles) sort_and_publish(kc + 1);
