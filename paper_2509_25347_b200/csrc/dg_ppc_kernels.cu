@@ -237,12 +237,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             {
                 // the fields travel into the (still unused) table: t_s -> col 2, rho_d -> col 3 of my own rows, rho_g ->
                 // my copy of the zz slot; a lane reads back only what it requested itself
-                static_for<0, g>([&](auto a) {
-                    const int k = 2 * a + r;    // dust species at my own position a (an inert slot re-reads species 0)
-                    const long long row = (long long)(k < N ? k : 0) * nc + cell;
-                    cp_async8(&Core::at(V, 2 * a, 2), G.t_s + row);
-                    cp_async8(&Core::at(V, 2 * a, 3), G.rho_d + row);
-                });
+                {
+                    // my own positions hold the dust species k = 2a + r: rows r, r + 2, ... of t_s and rho_d (running
+                    // pointers; an inert slot re-reads the last live row)
+                    const double* pt = G.t_s + (long long)r * nc + cell;
+                    const double* pd = G.rho_d + (long long)r * nc + cell;
+                    const long long step = 2 * nc;
+                    static_for<0, g>([&](auto a) {
+                        cp_async8(&Core::at(V, 2 * a, 2), pt);
+                        cp_async8(&Core::at(V, 2 * a, 3), pd);
+                        if (2 * (a + 1) + r < N) {
+                            pt += step;
+                            pd += step;
+                        }
+                    });
+                }
                 cp_async8(&V.x[Core::ZZ * CW], G.rho_g + cell);  // (an absent cell reads the tile's first cell)
                 cp_async_wait_all();
                 double ts[g], rd[g];
