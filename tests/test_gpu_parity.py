@@ -325,6 +325,35 @@ def test_pointers_that_are_8_but_not_16_byte_aligned(dg, oracle, cuda, N, varian
         assert torch.equal(args[4], ref_dev), which
 
 
+@pytest.mark.parametrize("N", [13, 16])
+def test_pair_per_cell_scheduler_with_wildly_uneven_tiles(dg, oracle, cuda, N):
+    """The pair-per-cell kernel hands out chunks of sorted 128-cell tiles to its warps through a small lock-free queue
+    (three order buffers per block).  Whole tiles of trivially cheap cells (dt/t_s ~ 1e-9: s = 0, m = 2) next to tiles of
+    very stiff ones (dt/t_s ~ 1e8: s ~ 30) make some warps fall several tiles behind the others — the situation in which a
+    lagging warp meets a recycled buffer.  Few enough cells that one block walks many tiles.  Must terminate, match the
+    oracle where it can referee (||A||_1 <= 1e6) and conserve momentum everywhere."""
+    ncells = 128 * 61 + 37
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
+    tile = torch.arange(ncells, device=cuda) // 128
+    cheap = (tile % 3 != 1)
+    stiff = (tile % 7 == 1)
+    wl.t_s[:, cheap] = 1e7
+    wl.t_s[:, stiff] = 1e-10
+    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    torch.cuda.synchronize()
+    assert int(s.max()) >= 25 and int(s.min()) == 0
+    rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(ncells))
+    got = out.cpu().numpy()
+    assert np.isfinite(got).all()
+    assert float(oracle.conservation_error(got, p_in).max()) <= CONS_TOL
+    norm = 2.0 * np.maximum((rho_d / rho_g * wl.dt / t_s).sum(axis=0), (wl.dt / t_s).max(axis=0))
+    ok = norm <= 1e6
+    ref = oracle.drag_update(rho_g[ok], rho_d[:, ok], t_s[:, ok], wl.dt, p_in[:, :, ok])
+    assert float(oracle.parity_error(got[:, :, ok], ref, p_in[:, :, ok]).max()) <= PARITY_TOL
+    again = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    assert torch.equal(again, out)               # deterministic whatever the order in which the warps claimed chunks
+
+
 @pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
 @pytest.mark.parametrize("variant", [0, 1, 2, 4])
 def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
