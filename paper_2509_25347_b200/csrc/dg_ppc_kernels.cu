@@ -376,27 +376,39 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                 double pa[3], pb[3];
                 load_p(0, pa);
                 load_p(g > 1 ? 1 : 0, pb);
-#pragma unroll 1
-                for (int a = 0; a < g; ++a) {
-                    double pc[3], y[3];
-                    static_for<0, 3>([&](auto cp) {
-                        pc[cp] = pa[cp];
-                        pa[cp] = pb[cp];
-                    });
-                    load_p(a + 2 < g ? a + 2 : g - 1, pb);
-                    Core::apply_row(V, c_tab.ap[a], q, q0, y);
+                auto row = [&](int a, const double (&pc)[3], const double (&y)[3]) {
                     const double w = V.x[((2 * a) * Core::ROW + Core::CWT) * CW];
                     if (valid && 2 * a + r < N) {
                         static_for<0, 3>([&](auto cp) { pout[cp * comp_stride] = fma(w, y[cp], pc[cp]); });
                     }
                     pout += 2 * nc;
+                };
+                // two rows per iteration: twelve independent FMA chains instead of six
+#pragma unroll 1
+                for (int a = 0; a + 1 < g; a += 2) {
+                    double pc0[3], pc1[3], y0[3], y1[3];
+                    static_for<0, 3>([&](auto cp) {
+                        pc0[cp] = pa[cp];
+                        pc1[cp] = pb[cp];
+                    });
+                    load_p(a + 2 < g ? a + 2 : g - 1, pa);
+                    load_p(a + 3 < g ? a + 3 : g - 1, pb);
+                    Core::apply_row(V, c_tab.ap[a], q, q0, y0);
+                    Core::apply_row(V, c_tab.ap[a + 1], q, q0, y1);
+                    row(a, pc0, y0);
+                    row(a + 1, pc1, y1);
+                }
+                if constexpr (g % 2 == 1) {
+                    double y[3];
+                    Core::apply_row(V, c_tab.ap[g - 1], q, q0, y);
+                    row(g - 1, pa, y);
                 }
                 {  // the gas row (both lanes compute it, role 0 stores it)
                     double y[3];
                     Core::apply_row(V, c_tab.ap[g], q, q0, y);
                     if (valid && r == 0) {
                         static_for<0, 3>([&](auto cp) {
-                            G.p_out[cp * comp_stride + cell] = G.p_in[cp * comp_stride + cell] + y[cp];
+                            G.p_out[cp * comp_stride + cell] = q0[cp] + y[cp];  // q0 is the gas momentum itself (w_z = 1)
                         });
                     }
                 }
