@@ -340,21 +340,38 @@ def bench_rk1(dg, wl, p_out, hbm_gbs, steps=5, warmup=3):
 
 
 def bench_paper_variant(dg, wl, p_out, steps=2, warmup=1):
-    """The paper's own scheme as printed (DG_VARIANT_PAPER: one thread per cell, dense matrices, Alg. 7 + plain
-    squarings) on the same buffers, for the design comparison on the same hardware."""
-    f = lambda: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=dg.DG_VARIANT_PAPER)
-    for _ in range(warmup):
-        f()
-    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(steps):
-        f()
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / steps
+    """The paper's own scheme as printed (one thread per cell, dense matrices, Alg. 7 + plain squarings; SURVEY.md
+    §8(f) rank 3) on the same buffers, for the design comparison on the same hardware: with the row chosen by
+    min(Pi_m + s) (DG_VARIANT_PAPER), by Algorithm 2 as printed (DG_VARIANT_PAPER_ALG2), and with Algorithm 2 plus the
+    bound test of Algorithms 8-9 (DG_VARIANT_PAPER_BOUND: products saved per cell = (m - m_evaluated) / q)."""
+    def timed(variant):
+        f = lambda: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=variant)
+        for _ in range(warmup):
+            f()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            _, s, m = f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps, s, m
+    ms, s0, m0 = timed(dg.DG_VARIANT_PAPER)
     drift = ((p_out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)).max().item()
-    return {"ms_per_launch": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "max_momentum_drift": drift}
+    res = {"ms_per_launch": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "max_momentum_drift": drift}
+    pi = {2: 1, 4: 2, 6: 3, 9: 4, 12: 5, 16: 6, 20: 7, 25: 8, 30: 9}
+    qq = {2: 1, 4: 2, 6: 2, 9: 3, 12: 3, 16: 4, 20: 4, 25: 5, 30: 5}
+    pi_t = torch.zeros(31, dtype=torch.float64, device=s0.device); q_t = torch.ones(31, dtype=torch.float64, device=s0.device)
+    for k, v in pi.items():
+        pi_t[k] = v; q_t[k] = qq[k]
+    cost = lambda s, m: float((pi_t[m.long()] + s.double()).mean().item())
+    res["mean_products_min_cost"] = cost(s0, m0)
+    ms2, s2, m2 = timed(dg.DG_VARIANT_PAPER_ALG2)
+    res["alg2"] = {"ms_per_launch": ms2, "mean_products": cost(s2, m2)}
+    ms3, s3, m3 = timed(dg.DG_VARIANT_PAPER_BOUND)
+    saved = ((m2 - m3).double() / q_t[m2.long()]).mean().item()
+    res["alg2_bound_test"] = {"ms_per_launch": ms3, "mean_products_saved_by_bound_test": float(saved)}
+    return res
 
 
 def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):

@@ -123,12 +123,19 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
  *                       (N+1)x(N+1) fp64 matrices, Table B.1 row minimising Pi_m + s on ||A||_1 (Eq. B.11), Taylor
  *                       polynomial by Algorithm 7, plain squarings (Alg. 6).  A measured reference for the design
  *                       comparison; its error grows like 2^s u on stiff cells.
+ *   DG_VARIANT_PAPER_ALG2   as DG_VARIANT_PAPER with (m, s) chosen by the paper's Algorithm 2 as printed
+ *                       (the branch-reduced "first modification" of Sastre et al.)
+ *   DG_VARIANT_PAPER_BOUND  as DG_VARIANT_PAPER_ALG2 plus the "second modification": the bound b_exp by Algorithm 8
+ *                       and the evaluation with bound test by Algorithm 9; m_out then
+ *                       reports the degree actually evaluated, m - q * (blocks the test dropped)
  * Any other value is DG_EINVAL. */
 #define DG_VARIANT_DEFAULT 0
 #define DG_VARIANT_TPC 1
 #define DG_VARIANT_WPC 2
 #define DG_VARIANT_PAPER 3
 #define DG_VARIANT_PPC 4
+#define DG_VARIANT_PAPER_ALG2 5
+#define DG_VARIANT_PAPER_BOUND 6
 dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                  const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                                  int variant, void* stream);

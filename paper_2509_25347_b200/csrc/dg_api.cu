@@ -63,7 +63,9 @@ static dg_status check_common(int N, long long ncells, bool* noop) {
 
 cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st) {
     if (variant == DG_VARIANT_DEFAULT) variant = default_variant(N);
-    if (variant == DG_VARIANT_PAPER) return kPaperTable[N]->update(a, st);
+    if (variant == DG_VARIANT_PAPER) return kPaperTable[N]->update[0](a, st);
+    if (variant == DG_VARIANT_PAPER_ALG2) return kPaperTable[N]->update[1](a, st);
+    if (variant == DG_VARIANT_PAPER_BOUND) return kPaperTable[N]->update[2](a, st);
     if (variant == DG_VARIANT_PPC) return kPpcTable[N]->update(a, N, st);
     return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
 }
@@ -131,7 +133,7 @@ dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const
     dg_status st = check_common(N, ncells, &noop);
     if (st != DG_OK) return st;
     if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
-    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PPC) return DG_EINVAL;
+    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PAPER_BOUND) return DG_EINVAL;
     if (noop) return DG_OK;
     DG_CHECK_PTR(rho_g);
     DG_CHECK_PTR(rho_d);

@@ -55,7 +55,7 @@ struct WpcLaunchers {
 
 // The paper's scheme as printed (dg_paper_kernels.cu, one translation unit per N): a measured reference, not the product.
 struct PaperLaunchers {
-    cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    cudaError_t (*update[3])(const UpdateArgs&, cudaStream_t);  // [0] min(Pi_m + s); [1] Alg. 2; [2] Alg. 2 + Alg. 8/9
     const char* variant;
 };
 

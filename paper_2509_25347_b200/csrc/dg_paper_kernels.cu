@@ -11,6 +11,18 @@
 //      F <- (B_k + F) A^q for k >= 1, F <- B_0 + F for k = 0, finally F += b_0 I;
 //   4. s plain squarings F <- F F (Alg. 6 step 3);
 //   5. p_out = F p_in (Eq. 18).
+// Three modes (template parameter MODE, one kernel each):
+//   0  DG_VARIANT_PAPER        row by min(Pi_m + s), Alg. 7                     (what round 1 built)
+//   1  DG_VARIANT_PAPER_ALG2   row and s by Algorithm 2 AS PRINTED (the branch-reduced rewrite of
+//                              Alg. 1 option 2: Sastre et al.'s "first modification"), then Alg. 7.  Readings (DESIGN.md
+//                              R8): line 4 reads s* = s^ (as printed, "s* = 0", nothing would ever be scaled); k^ is the k
+//                              at which the loop stopped, K if it never did; lines 17-21 apply only if v > 0 (with
+//                              v1 = v2 = v3 = 0 the printed test "v = v1" holds and would cut a product for nothing).
+//   2  DG_VARIANT_PAPER_BOUND  Alg. 2, then the "second modification": the bound b_exp ~ ||exp(-A)|| by Algorithm 8
+//                              (Eq. B.17) and the evaluation with bound test by Algorithm 9
+//                              (Eq. B.15-B.18): a block whose contribution b_exp ||B_k + F|| ||A^q||^k
+//                              is below u is dropped instead of multiplied by A^q (F = 0: Alg. 5's "F = B_{j-1}",
+//                              PAPER.md:856-858, in merged form).  m_out reports q r - q (blocks dropped).
 // Plain fp64 scaling and squaring: the error along the conserved mode grows like 2^s u, so this variant
 // meets the paper's own accuracy level (Er_1 ~ 1e-8), not BASELINE.json's 1e-12 on the stiff configs; the
 // tests hold it to what it can deliver and DESIGN.md §7 reports the measured figures beside the product path's.
@@ -47,6 +59,56 @@ __device__ __forceinline__ void matmul(const double (&X)[NN], const double (&Y)[
         }
 }
 
+// ||X||_1: largest column sum of |X_ik|
+__device__ __forceinline__ double norm1(const double (&X)[NN]) {
+    double nrm = 0.0;
+#pragma unroll kUnroll
+    for (int k = 0; k < n; ++k) {
+        double col = 0.0;
+#pragma unroll
+        for (int i = 0; i < n; ++i) col += fabs(X[i * n + k]);
+        nrm = fmax(nrm, col);
+    }
+    return nrm;
+}
+
+// Algorithm 2, as printed with the three readings in the header.  k = 1..K = 9 are the rows of
+// Table B.1 (row index k - 1).  Branch-free but for the final selects, as the paper intends.
+__device__ __forceinline__ void algorithm2(double norm, int& row, int& s) {
+    constexpr int K = kRows;
+    const double thK = c_theta[K - 1];
+    const int shat = scaling_exponent(norm, thK);  // ceil(max(log2(||A|| / theta_mK), 0)), exactly
+    int kstar = K;
+    bool cond = false;
+#pragma unroll
+    for (int k = 1; k <= K; ++k) {
+        const bool hit = !cond && norm <= fmin(c_theta[k - 1], thK);
+        kstar = hit ? k : kstar;
+        cond = cond || hit;
+    }
+    const int khat = kstar;
+    const double cmp = norm * pow2neg(min(shat, kSMax));
+    const int v1 = (khat >= 7 && cmp <= c_theta[max(khat - 2, 0)]) ? 1 : 0;
+    const int v2 = (khat >= 8 && cmp <= 2.0 * c_theta[max(khat - 3, 0)]) ? 2 : 0;
+    const int v3 = (khat >= 9 && cmp <= 4.0 * c_theta[max(khat - 4, 0)]) ? 3 : 0;
+    const int v = max(v1, max(v2, v3));
+    int sstar = shat;
+    if (v > 0) {
+        if (v == v1) {
+            kstar = khat - 1;
+        } else if (v == v2) {
+            kstar = khat - 2;
+            sstar = max(1, shat + 1);
+        } else {
+            kstar = khat - 3;
+            sstar = max(2, shat + 2);
+        }
+    }
+    row = kstar - 1;
+    s = sstar;
+}
+
+template <int MODE>
 __global__ void __launch_bounds__(kThreads) k_update_paper(UpdateArgs g) {
     const long long c = (long long)blockIdx.x * kThreads + threadIdx.x;
     const long long nc = g.ncells;
@@ -80,25 +142,59 @@ __global__ void __launch_bounds__(kThreads) k_update_paper(UpdateArgs g) {
     }
     int row = kRows - 1, s = 0;
     if (norm <= 1.7e308) {
-        int best = 0x7fffffff;
+        if constexpr (MODE == 0) {
+            int best = 0x7fffffff;
 #pragma unroll
-        for (int k = 0; k < kRows; ++k) {
-            const int sk = scaling_exponent(norm, c_theta[k]);
-            const int cost = (c_q[k] + c_r[k] - 2) + sk;
-            if (cost < best) { best = cost; row = k; s = sk; }
+            for (int k = 0; k < kRows; ++k) {
+                const int sk = scaling_exponent(norm, c_theta[k]);
+                const int cost = (c_q[k] + c_r[k] - 2) + sk;
+                if (cost < best) { best = cost; row = k; s = sk; }
+            }
+        } else {
+            algorithm2(norm, row, s);
         }
         s = min(s, kSMax);
     }
     const int q = c_q[row], r = c_r[row];
     if (g.s_out) g.s_out[c] = s;
-    if (g.m_out) g.m_out[c] = q * r;
     {
         const double sc = pow2neg(s);
 #pragma unroll
         for (int k = 0; k < NN; ++k) A[k] *= sc;
     }
-    // 3. Algorithm 7
     double F[NN], T[NN];
+    // 3'. Algorithm 8: b_exp, the bound of ||exp(-A)|| (Eq. B.17), powers recomputed block by block, b_i = (-1)^i / i!
+    double bexp = 0.0;
+    if constexpr (MODE == 2) {
+#pragma unroll 1
+        for (int l = r - 1; l >= 0; --l) {
+            double P[NN];
+#pragma unroll
+            for (int e = 0; e < NN; ++e) {
+                P[e] = A[e];
+                F[e] = (((q * l + 1) & 1) ? -c_ifact[q * l + 1] : c_ifact[q * l + 1]) * P[e];   // B^_l, j = 1
+            }
+#pragma unroll 1
+            for (int j = 2; j <= q; ++j) {
+                matmul(A, P, T);
+                const double b = ((q * l + j) & 1) ? -c_ifact[q * l + j] : c_ifact[q * l + j];
+#pragma unroll
+                for (int e = 0; e < NN; ++e) {
+                    P[e] = T[e];
+                    F[e] = fma(b, P[e], F[e]);
+                }
+            }
+            if (l >= 1) {
+                bexp = (norm1(F) + bexp) * norm1(P);
+            } else {
+#pragma unroll
+                for (int i = 0; i < n; ++i) F[i * n + i] += 1.0;   // b_0 I + B^_0
+                bexp += norm1(F);
+            }
+        }
+    }
+    int dropped = 0;
+    // 3. Algorithm 7 (MODE 0, 1) / Algorithm 9 (MODE 2: the same with the bound test)
 #pragma unroll
     for (int k = 0; k < NN; ++k) F[k] = 0.0;
 #pragma unroll 1
@@ -119,11 +215,25 @@ __global__ void __launch_bounds__(kThreads) k_update_paper(UpdateArgs g) {
             }
         }
         if (k >= 1) {                                                   // F <- (B_k + F) A^q
-            matmul(F, P, T);
+            bool drop = false;
+            if constexpr (MODE == 2) {                                  // cond_2: b_exp ||B_k + F|| ||A^q||^k <= u
+                const double nq = norm1(P);
+                double pw = nq;
+                for (int e = 1; e < k; ++e) pw *= nq;
+                drop = bexp * norm1(F) * pw <= 1.1102230246251565e-16;
+            }
+            if (drop) {
+                ++dropped;
 #pragma unroll
-            for (int e = 0; e < NN; ++e) F[e] = T[e];
+                for (int e = 0; e < NN; ++e) F[e] = 0.0;
+            } else {
+                matmul(F, P, T);
+#pragma unroll
+                for (int e = 0; e < NN; ++e) F[e] = T[e];
+            }
         }
     }
+    if (g.m_out) g.m_out[c] = q * r - q * dropped;
 #pragma unroll
     for (int i = 0; i < n; ++i) F[i * n + i] += 1.0;                    // + b_0 I
     // 4. squarings
@@ -149,8 +259,9 @@ __global__ void __launch_bounds__(kThreads) k_update_paper(UpdateArgs g) {
     }
 }
 
+template <int MODE>
 cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    k_update_paper<<<(unsigned)((a.ncells + kThreads - 1) / kThreads), kThreads, 0, st>>>(a);
+    k_update_paper<MODE><<<(unsigned)((a.ncells + kThreads - 1) / kThreads), kThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
@@ -159,6 +270,7 @@ cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
 #define DG_CAT_(a, b) a##b
 #define DG_CAT(a, b) DG_CAT_(a, b)
 extern const PaperLaunchers DG_CAT(paper_launchers_N, DG_N) = {
-    launch_update, "paper as printed: thread-per-cell, dense Alg. 7 + plain squarings"};
+    {launch_update<0>, launch_update<1>, launch_update<2>},
+    "paper as printed: thread-per-cell, dense Alg. 7 + plain squarings"};
 
 }  // namespace dg

@@ -121,6 +121,74 @@ def test_paper_as_printed_variant(dg, oracle, cuda, N):
     assert torch.equal(out0, wl.p_in)
 
 
+THETA = [2.5809568029e-8, 3.3971688399e-4, 9.0656564075e-3, 8.9577602032e-2, 2.9961589138e-1, 7.8028742566e-1,
+         1.4382525967, 2.4285825244, 3.5396663487]     # Table B.1, rows 5-6 recomputed (R3)
+M_OF_ROW = [2, 4, 6, 9, 12, 16, 20, 25, 30]
+
+
+def algorithm2_as_printed(norm):
+    """Algorithm 2 of the paper retyped line by line for one norm, with DESIGN.md R8's readings:
+    line 4 is s* = s^, k^ is the k at which the loop stopped (K if it never did), lines 17-21 need v > 0."""
+    K = 9
+    shat = int(max(np.ceil(np.log2(norm / THETA[K - 1])), 0)) if norm > 0 else 0
+    while norm / 2.0 ** shat > THETA[K - 1]:            # (guards the rounded log2 at the thresholds)
+        shat += 1
+    while shat > 0 and norm / 2.0 ** (shat - 1) <= THETA[K - 1]:
+        shat -= 1
+    mstar, kstar, sstar, cond = M_OF_ROW[K - 1], K, shat, False
+    for k in range(1, K + 1):
+        if cond:
+            break
+        cond = norm <= min(THETA[k - 1], THETA[K - 1])
+        if cond:
+            mstar, kstar = M_OF_ROW[k - 1], k
+    khat = kstar
+    cmp_ = norm / 2.0 ** shat
+    v1 = 1 if (khat >= 7 and cmp_ <= THETA[khat - 2]) else 0
+    v2 = 2 if (khat >= 8 and cmp_ <= 2 * THETA[khat - 3]) else 0
+    v3 = 3 if (khat >= 9 and cmp_ <= 4 * THETA[khat - 4]) else 0
+    v = max(v1, v2, v3)
+    if v > 0:
+        if v == v1:
+            kstar = khat - 1
+        elif v == v2:
+            kstar, sstar = khat - 2, max(1, shat + 1)
+        else:
+            kstar, sstar = khat - 3, max(2, shat + 2)
+        mstar = M_OF_ROW[kstar - 1]
+    return mstar, sstar
+
+
+@pytest.mark.parametrize("N", [1, 2, 4, 8, 12, 16])
+def test_paper_algorithm2_and_bound_test_variants(dg, oracle, cuda, N):
+    """SURVEY.md 8(f) rank 3, second half: DG_VARIANT_PAPER_ALG2 chooses (m, s) by the paper's Algorithm 2 as printed —
+    compared here with a line-by-line retyping — and DG_VARIANT_PAPER_BOUND adds Algorithms 8 and 9 (the bound test of
+    Eq. B.15-B.18).  Both are plain scaling and squaring and are held to what that delivers, like DG_VARIANT_PAPER."""
+    for cfg, tol in ((5, 1e-9), (2, 1e-12)):
+        wl = W.make_workload(cfg, ncells=1200 + 11 * N, N=N, device=cuda)
+        rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(wl.ncells))
+        ref = oracle.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+        a = wl.dt / t_s
+        norm1 = 2.0 * np.maximum((rho_d / rho_g[None, :] * a).sum(axis=0), a.max(axis=0))
+        out2, s2, m2 = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=dg.DG_VARIANT_PAPER_ALG2)
+        out3, s3, m3 = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=dg.DG_VARIANT_PAPER_BOUND)
+        s2, m2, s3, m3 = (x.cpu().numpy() for x in (s2, m2, s3, m3))
+        for out in (out2, out3):
+            got = out.cpu().numpy()
+            assert np.isfinite(got).all()
+            assert float(oracle.parity_error(got, ref, p_in).max()) <= tol
+            assert float(oracle.conservation_error(got, p_in).max()) <= tol
+        # Algorithm 2's choice, cell by cell (the kernel sums the columns in fp64 in its own order: a norm within a
+        # few ulp of a threshold may fall on the other side)
+        expect = np.array([algorithm2_as_printed(float(x)) for x in norm1])
+        agree = (expect[:, 0] == m2) & (expect[:, 1] == s2)
+        assert agree.mean() >= 0.995, (N, cfg, agree.mean())
+        th = np.array([THETA[M_OF_ROW.index(int(k))] for k in m2])
+        assert (norm1 / 2.0 ** s2 <= th * (1 + 1e-9)).all()          # Theorem 1's premise for Alg. 2's (m, s)
+        # the bound test only ever drops whole blocks of q terms from the top, and never changes s
+        assert (s3 == s2).all() and (m3 <= m2).all() and (m3 >= 0).all()
+
+
 # ------------------------------------------------------------------ full sizes, the launch configuration bench.py times
 @pytest.mark.parametrize("config", [2, 3, 4])
 def test_full_size_sampled(dg, oracle, cuda, config):
