@@ -294,5 +294,65 @@ int dgo_rk1_update(const double *rho_g, const double *rho_d, const double *t_s, 
     return bad;
 }
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * Gas energy over one exact drag step: frictional heating (Eq. 4 and the third entry of Eq. 11).
+ * With the transport and external-force terms split off (Eq. 25-26) the gas energy obeys
+ *     dE_g/dt = sum_i rho_d,i (v_d,i - v_g)/T_s,i . v_g  +  w sum_i rho_d,i (v_d,i - v_g)^2 / T_s,i        (w in [0, 1])
+ * along the exact solution p(t) = exp(t Omega) p(0) of the momenta (Eq. 18).  The paper gives NO discrete formula for
+ * it (reading R20); what is computed here is the exact integral of that equation over the step:
+ *   - the first term is v_g . dM_g/dt = d/dt (|M_g|^2 / (2 rho_g))     (rho_g is constant during the drag step),
+ *   - the second is  -w dK/dt  with  K = |M_g|^2/(2 rho_g) + sum_i |M_d,i|^2/(2 rho_d,i)  the total kinetic energy,
+ *     because  dK/dt = v_g . dM_g/dt + sum_i v_d,i . dM_d,i/dt = - sum_i rho_d,i (v_d,i - v_g)^2 / T_s,i  by Eq. 3, 6;
+ *   hence     E_g(t+dt) = E_g(t) + [KE_g(t+dt) - KE_g(t)] + w [K(t) - K(t+dt)],
+ *   with the momenta at t+dt from the oracle's own exponential.  w = 1: E_g + sum_i |M_d,i|^2/(2 rho_d,i) is conserved.
+ * A species with rho_d,i = 0 carries no momentum and no energy (its term is skipped).
+ * Pins (tests/test_energy.py): the heating integral by 30-digit quadrature of the second term along the exact
+ * trajectory (mpmath, Eq. 4 retyped), and the N = 1 closed form  mu |dv_0|^2 (1 - exp(-2 kappa dt)) / 2.
+ * p_out (nullable) receives the momenta after the step. */
+int dgo_energy_update(const double *rho_g, const double *rho_d, const double *t_s, double dt, const double *p_in,
+                      const double *E_in, double w, int N, long long ncells, ld *E_out, ld *p_out, int nthreads)
+{
+    if (check_args(N, ncells)) return 1;
+    int n = N + 1;
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#endif
+#pragma omp parallel
+    {
+        ld *A = (ld *)malloc(sizeof(ld) * (5 * n * n + 6 * n));
+        ld *E = A + n * n, *work = A + 2 * n * n, *pi = A + 5 * n * n, *po = pi + 3 * n;
+        double rd[DGO_NMAX], ts[DGO_NMAX];
+#pragma omp for schedule(dynamic, 64)
+        for (long long c = 0; c < ncells; ++c) {
+            for (int i = 0; i < N; ++i) { rd[i] = rho_d[(long long)i * ncells + c]; ts[i] = t_s[(long long)i * ncells + c]; }
+            dgo_cell_matrix(rho_g[c], rd, ts, dt, N, A);
+            dgo_expm(A, n, E, work);
+            for (int k = 0; k < 3 * n; ++k) pi[k] = (ld)p_in[(long long)k * ncells + c];
+            dgo_cell_apply(E, pi, n, po);
+            ld keg_in = 0.0L, keg_out = 0.0L, kd_in = 0.0L, kd_out = 0.0L;
+            for (int comp = 0; comp < 3; ++comp) {
+                keg_in += pi[comp * n] * pi[comp * n];
+                keg_out += po[comp * n] * po[comp * n];
+            }
+            keg_in /= 2.0L * (ld)rho_g[c];
+            keg_out /= 2.0L * (ld)rho_g[c];
+            for (int i = 1; i <= N; ++i) {
+                if (rd[i - 1] == 0.0) continue;
+                ld a = 0.0L, b = 0.0L;
+                for (int comp = 0; comp < 3; ++comp) {
+                    a += pi[comp * n + i] * pi[comp * n + i];
+                    b += po[comp * n + i] * po[comp * n + i];
+                }
+                kd_in += a / (2.0L * (ld)rd[i - 1]);
+                kd_out += b / (2.0L * (ld)rd[i - 1]);
+            }
+            E_out[c] = (ld)E_in[c] + (keg_out - keg_in) + (ld)w * ((keg_in + kd_in) - (keg_out + kd_out));
+            if (p_out) for (int k = 0; k < 3 * n; ++k) p_out[(long long)k * ncells + c] = po[k];
+        }
+        free(A);
+    }
+    return 0;
+}
+
 int dgo_sizeof_long_double(void) { return (int)sizeof(ld); }
 int dgo_ldbl_mant_dig(void) { return __LDBL_MANT_DIG__; }

@@ -113,6 +113,22 @@ def rk1_update(rho_g, rho_d, t_s, dt, p_in, nthreads=0):
     return out
 
 
+def energy_update(rho_g, rho_d, t_s, dt, p_in, E_in, w, nthreads=0):
+    """Gas energy after one exact drag step with frictional heating (Eq. 4; R20): returns
+    (E_out longdouble [ncells], p_out longdouble [3][n][ncells])."""
+    N = rho_d.shape[0]
+    rho_g, prg = _f64(rho_g); rho_d, prd = _f64(rho_d); t_s, pts = _f64(t_s); p_in, pp = _f64(p_in); E_in, pe = _f64(E_in)
+    ncells = _shape_check(rho_g, rho_d, t_s, N)
+    n = N + 1
+    assert p_in.shape == (3, n, ncells) and E_in.shape == (ncells,)
+    E_out = np.empty(ncells, dtype=LD)
+    p_out = np.empty((3, n, ncells), dtype=LD)
+    rc = lib().dgo_energy_update(prg, prd, pts, C.c_double(dt), pp, pe, C.c_double(w), C.c_int(N), C.c_longlong(ncells),
+                                 E_out.ctypes.data_as(C.c_void_p), p_out.ctypes.data_as(C.c_void_p), C.c_int(nthreads))
+    assert rc == 0
+    return E_out, p_out
+
+
 def parity_error(p_gpu, p_ref, p_in):
     """DESIGN.md reading R13: per cell, max_{k,comp}|p_gpu - p_ref| / max_{k,comp}|p_in|, in long double."""
     d = np.abs(np.asarray(p_gpu, dtype=LD) - np.asarray(p_ref, dtype=LD)).reshape(-1, p_ref.shape[-1]).max(axis=0)
