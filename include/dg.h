@@ -112,6 +112,20 @@ dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const d
 dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,
                       int N, long long ncells, double* p_out, void* stream);
 
+/* ---- drag update + gas energy with frictional heating  (Eq. 4 and Eq. 11) ----------------------
+ * p_out as dg_drag_update, and the gas total energy E_g = |M_g|^2/(2 rho_g) + e after the drag step:
+ *     E_out = E_in + [KE_g(p_out) - KE_g(p_in)] + w * [K(p_in) - K(p_out)],
+ * K = |M_g|^2/(2 rho_g) + sum_i |M_d,i|^2/(2 rho_d,i) the total kinetic energy of the cell.  This is Eq. 4's drag part
+ * integrated exactly along the exact momenta (the paper prints no discrete formula; reading R20): the first
+ * bracket is the work of the drag force on the gas, the second the kinetic energy the drag dissipates, of which the
+ * fraction w (0 = no frictional heating, 1 = all of it) is deposited into the gas.  With w = 1,
+ * E_g + sum_i |M_d,i|^2/(2 rho_d,i) is conserved.  A species with rho_d,i = 0 carries no energy.
+ * in : rho_g, rho_d, t_s, p_in, E_in [ncells] (device), dt, w.   out: p_out (may alias p_in), E_out [ncells] (may alias
+ * E_in).  Three launches on `stream`.  DG_EINVAL if w is outside [0, 1]; otherwise the errors of dg_drag_update. */
+dg_status dg_drag_update_energy(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                                const double* p_in, const double* E_in, double w, int N, long long ncells,
+                                double* p_out, double* E_out, void* stream);
+
 /* Same as dg_drag_update_ex with the thread mapping forced (for measuring the mappings against each other; both
  * compute the same arithmetic and agree to rounding):
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)

@@ -19,7 +19,7 @@ DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
  DG_VARIANT_PAPER_BOUND) = range(7)
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
-           "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1",
+           "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy",
            "dg_drag_update_host", "dg_host_release", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
            "dg_status_string", "dg_last_cuda_error", "dg_version")
 
@@ -47,6 +47,7 @@ def _load():
     lib.dg_drag_update_variant.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp, vp, i32, vp]
     lib.dg_drag_update_steps.argtypes = [vp, vp, vp, dbl, vp, i32, ll, i32, vp, vp]
     lib.dg_drag_rk1.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
+    lib.dg_drag_update_energy.argtypes = [vp, vp, vp, dbl, vp, vp, dbl, i32, ll, vp, vp, vp]
     lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
     lib.dg_host_release.argtypes = []
     lib.dg_peak_kernel.argtypes = [i32, i32, vp, ll, C.POINTER(dbl), vp]
@@ -185,6 +186,22 @@ def dg_drag_rk1(rho_g, rho_d, t_s, dt, p_in, p_out=None):
                           _dev(p_out, "p_out", (3, n, ncells)), _stream())
     _check(st, "dg_drag_rk1")
     return p_out
+
+
+def dg_drag_update_energy(rho_g, rho_d, t_s, dt, p_in, E_in, w, p_out=None, E_out=None):
+    """Fused drag update plus the gas energy with frictional heating (Eq. 4; w in [0, 1]): returns (p_out, E_out)."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    if E_out is None:
+        E_out = torch.empty_like(E_in)
+    st = _lib.dg_drag_update_energy(_dev(rho_g, "rho_g", (ncells,)), _dev(rho_d, "rho_d", (N, ncells)),
+                                    _dev(t_s, "t_s", (N, ncells)), float(dt), _dev(p_in, "p_in", (3, n, ncells)),
+                                    _dev(E_in, "E_in", (ncells,)), float(w), N, ncells,
+                                    _dev(p_out, "p_out", (3, n, ncells)), _dev(E_out, "E_out", (ncells,)), _stream())
+    _check(st, "dg_drag_update_energy")
+    return p_out, E_out
 
 
 def _host(t, name, shape):

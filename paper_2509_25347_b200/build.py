@@ -4,7 +4,7 @@
 
 One object per translation unit, compiled in parallel: dg_kernels.cu, dg_wpc_kernels.cu and dg_paper_kernels.cu once
 per species count N (-DDG_N=<N>), dg_ppc_kernels.cu once per even number of dust slots (-DDG_NP=<NP>), plus
-dg_api.cu, dg_peaks.cu, dg_host.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
+dg_api.cu, dg_peaks.cu, dg_host.cu, dg_energy.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
 nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 arithmetic must stay IEEE (the kernels' own Newton
 reciprocals are explicit, dg_params.cuh).  Extra nvcc flags for an experiment can be passed in DG_EXTRA_FLAGS.
 """
@@ -34,7 +34,8 @@ def _nvcc():
 
 def _units():
     """(object name, source, extra flags)"""
-    units = [("dg_api.o", "dg_api.cu", []), ("dg_peaks.o", "dg_peaks.cu", []), ("dg_host.o", "dg_host.cu", [])]
+    units = [("dg_api.o", "dg_api.cu", []), ("dg_peaks.o", "dg_peaks.cu", []), ("dg_host.o", "dg_host.cu", []),
+             ("dg_energy.o", "dg_energy.cu", [])]
     for n in range(1, NMAX + 1):
         units.append((f"dg_kernels_N{n}.o", "dg_kernels.cu", [f"-DDG_N={n}"]))
         units.append((f"dg_wpc_kernels_N{n}.o", "dg_wpc_kernels.cu", [f"-DDG_N={n}"]))
