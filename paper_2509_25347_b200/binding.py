@@ -19,7 +19,7 @@ DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
  DG_VARIANT_PAPER_BOUND) = range(7)
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
-           "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy",
+           "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy", "dg_drag_update_f32",
            "dg_drag_update_host", "dg_host_release", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
            "dg_status_string", "dg_last_cuda_error", "dg_version")
 
@@ -47,6 +47,7 @@ def _load():
     lib.dg_drag_update_variant.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp, vp, i32, vp]
     lib.dg_drag_update_steps.argtypes = [vp, vp, vp, dbl, vp, i32, ll, i32, vp, vp]
     lib.dg_drag_rk1.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
+    lib.dg_drag_update_f32.argtypes = [vp, vp, vp, C.c_float, vp, i32, ll, vp, vp, vp, vp]
     lib.dg_drag_update_energy.argtypes = [vp, vp, vp, dbl, vp, vp, dbl, i32, ll, vp, vp, vp]
     lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
     lib.dg_host_release.argtypes = []
@@ -202,6 +203,23 @@ def dg_drag_update_energy(rho_g, rho_d, t_s, dt, p_in, E_in, w, p_out=None, E_ou
                                     _dev(p_out, "p_out", (3, n, ncells)), _dev(E_out, "E_out", (ncells,)), _stream())
     _check(st, "dg_drag_update_energy")
     return p_out, E_out
+
+
+def dg_drag_update_f32(rho_g, rho_d, t_s, dt, p_in, p_out=None):
+    """The fused update in single precision (Eq. B.8 with u = 2^-24): float32 tensors in, (p_out, s, m) out."""
+    N, ncells = rho_d.shape
+    n = N + 1
+    f32 = torch.float32
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    s = torch.empty(ncells, dtype=torch.int32, device=rho_g.device)
+    m = torch.empty(ncells, dtype=torch.int32, device=rho_g.device)
+    st = _lib.dg_drag_update_f32(_dev(rho_g, "rho_g", (ncells,), f32), _dev(rho_d, "rho_d", (N, ncells), f32),
+                                 _dev(t_s, "t_s", (N, ncells), f32), float(dt), _dev(p_in, "p_in", (3, n, ncells), f32),
+                                 N, ncells, _dev(p_out, "p_out", (3, n, ncells), f32),
+                                 _dev(s, "s", (ncells,), torch.int32), _dev(m, "m", (ncells,), torch.int32), _stream())
+    _check(st, "dg_drag_update_f32")
+    return p_out, s, m
 
 
 def _host(t, name, shape):

@@ -26,6 +26,12 @@ static const PaperLaunchers* const kPaperTable[DG_NMAX + 1] = {
     &paper_launchers_N10, &paper_launchers_N11, &paper_launchers_N12, &paper_launchers_N13, &paper_launchers_N14,
     &paper_launchers_N15, &paper_launchers_N16};
 
+static const F32Launchers* const kF32Table[DG_NMAX + 1] = {
+    nullptr,            &f32_launchers_N1,  &f32_launchers_N2,  &f32_launchers_N3,  &f32_launchers_N4,
+    &f32_launchers_N5,  &f32_launchers_N6,  &f32_launchers_N7,  &f32_launchers_N8,  &f32_launchers_N9,
+    &f32_launchers_N10, &f32_launchers_N11, &f32_launchers_N12, &f32_launchers_N13, &f32_launchers_N14,
+    &f32_launchers_N15, &f32_launchers_N16};
+
 static const PpcLaunchers* const kPpcTable[DG_NMAX + 1] = {
     nullptr,
     &ppc_launchers_NP2,  &ppc_launchers_NP2,  &ppc_launchers_NP4,  &ppc_launchers_NP4,  &ppc_launchers_NP6,  &ppc_launchers_NP6,
@@ -175,6 +181,24 @@ dg_status dg_drag_update_steps(const double* rho_g, const double* rho_d, const d
     for (int k = 1; k < nsteps && st == DG_OK; ++k)
         st = dg_drag_update(rho_g, rho_d, t_s, dt, p_out, N, ncells, p_out, stream);
     return st;
+}
+
+dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float* t_s, float dt, const float* p_in,
+                             int N, long long ncells, float* p_out, int* s_out, int* m_out, void* stream) {
+    bool noop;
+    dg_status st = check_common(N, ncells, &noop);
+    if (st != DG_OK) return st;
+    if (!(dt >= 0.0f) || !std::isfinite(dt)) return DG_EINVAL;
+    if (noop) return DG_OK;
+    const void* ptrs[] = {rho_g, rho_d, t_s, p_in, p_out};
+    for (const void* p : ptrs) {
+        if (p == nullptr) return DG_ENULL;
+        if (reinterpret_cast<uintptr_t>(p) & 3u) return DG_EALIGN;
+    }
+    DG_CHECK_OPT_PTR(s_out);
+    DG_CHECK_OPT_PTR(m_out);
+    UpdateArgsF32 a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, s_out, m_out};
+    return cuda_status(kF32Table[N]->update(a, static_cast<cudaStream_t>(stream)));
 }
 
 dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_s, double dt, const double* p_in,

@@ -36,6 +36,18 @@ struct ApplyArgs {  // dg_drag_apply
     double* p_out;
 };
 
+struct UpdateArgsF32 {  // dg_drag_update_f32
+    const float* rho_g;
+    const float* rho_d;
+    const float* t_s;
+    float dt;
+    const float* p_in;
+    long long ncells;
+    float* p_out;
+    int* s_out;
+    int* m_out;
+};
+
 // One set of launchers per N (a translation unit each, compiled from dg_kernels.cu with -DDG_N=<N>).
 struct Launchers {
     cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
@@ -68,8 +80,14 @@ struct PpcLaunchers {
 extern const PpcLaunchers ppc_launchers_NP2, ppc_launchers_NP4, ppc_launchers_NP6, ppc_launchers_NP8, ppc_launchers_NP10,
     ppc_launchers_NP12, ppc_launchers_NP14, ppc_launchers_NP16;
 
+// Single-precision thread-per-cell kernel (dg_f32_kernels.cu, one translation unit per N).
+struct F32Launchers {
+    cudaError_t (*update)(const UpdateArgsF32&, cudaStream_t);
+};
+
 #define DG_DECL_LAUNCHERS(NN)                       \
     extern const Launchers launchers_N##NN;         \
+    extern const F32Launchers f32_launchers_N##NN;  \
     extern const WpcLaunchers wpc_launchers_N##NN;  \
     extern const PaperLaunchers paper_launchers_N##NN;
 DG_DECL_LAUNCHERS(1)

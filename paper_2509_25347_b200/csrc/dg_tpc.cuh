@@ -38,7 +38,7 @@ __device__ __forceinline__ void static_for(F&& f) {
     }
 }
 
-template <int N>
+template <int N, class Real = double>
 struct Tpc {
     static constexpr int n = N + 1;
     static constexpr int SZ = n * (n + 1) / 2;
@@ -53,18 +53,18 @@ struct Tpc {
     __host__ __device__ static constexpr float hcost() { return (float)kHornerOps / (float)kSquareOps; }
 
     // d_j = -(sum_{i != j} w_i O_ij) / w_j   (w_0 = 1); writes the diagonal slots of P.
-    __device__ __forceinline__ static void conserve(double (&P)[SZ], const double (&w)[N], const double (&iw)[N]) {
+    __device__ __forceinline__ static void conserve(Real (&P)[SZ], const Real (&w)[N], const Real (&iw)[N]) {
         static_for<0, n>([&](auto J) {
             constexpr int j = J;
             if constexpr (j == 0) {
-                double acc = w[0] * P[ix(0, 1)];
+                Real acc = w[0] * P[ix(0, 1)];
                 static_for<2, n>([&](auto I) {
                     constexpr int i = I;
                     acc = fma(w[i - 1], P[ix(0, i)], acc);
                 });
                 P[ix(0, 0)] = -acc;
             } else {
-                double acc = P[ix(0, j)];  // w_0 = 1
+                Real acc = P[ix(0, j)];  // w_0 = 1
                 static_for<1, n>([&](auto I) {
                     constexpr int i = I;
                     if constexpr (i != j) acc = fma(w[i - 1], P[sx(i, j)], acc);
@@ -85,25 +85,25 @@ struct Tpc {
     // scaling exponent and P holds X - I (packed, diagonal slots = d) with X = exp(S / 2^min(defer, s)): exp(S) itself
     // for defer = 0, the iterate min(defer, s) squarings short of it otherwise.
     template <int defer = 0>
-    __device__ __forceinline__ static void expm(const double (&a)[N], const double (&w)[N], const double (&iw)[N],
-                                                double (&P)[SZ], int& m, int& s) {
+    __device__ __forceinline__ static void expm(const Real (&a)[N], const Real (&w)[N], const Real (&iw)[N],
+                                                Real (&P)[SZ], int& m, int& s) {
         // The scaling exponent is chosen on ||S||_2 (Theorem 1, holds in any consistent norm; S is
         // symmetric and the whole iteration runs in S's basis).  S is negative semi-definite and its eigenvalues
         // -mu solve the secular equation 1 = sum_i eps_i a_i / (mu - a_i) (Eq. 29's lambda), whose
         // largest root obeys  mu <= max_i a_i + sum_i eps_i a_i  =: norm  (<= ||A||_1 = 2 max(sum eps a, max a);
         // DESIGN.md R5).
-        double sb = 0.0, amax = 0.0;
+        Real sb = Real(0), amax = Real(0);
         static_for<0, N>([&](auto I) {
             constexpr int i = I;
             sb = fma(a[i] * w[i], w[i], sb);
             amax = fmax(amax, a[i]);
         });
-        const double norm = sb + amax;
+        const Real norm = sb + amax;
         choose_m_s_warp(norm, hcost(), m, s);  // m is warp-uniform, s is this cell's own
-        const double sc = pow2neg(s);
+        const Real sc = Num<Real>::pow2(s);
 
-        double al[N], be[N];
-        double b00 = 0.0;
+        Real al[N], be[N];
+        Real b00 = Real(0);
         static_for<0, N>([&](auto I) {
             constexpr int i = I;
             al[i] = a[i] * sc;
@@ -125,14 +125,14 @@ struct Tpc {
         // The dust DIAGONAL is not carried at all: a step feeds P_ii only back into P_ii, and the final diagonal is
         // re-derived from conservation below.  P = Q_1 / m! is put back together at the end.
         // Storage: P[ix(0,k)] holds v_k, P[ix(i,k)] (1 <= i < k) holds U_ik, P[ix(0,0)] holds Q_00.
-        double be2[N];
+        Real be2[N];
         static_for<0, N>([&](auto I) { be2[I] = be[I] * be[I]; });
-        static_for<0, SZ>([&](auto K) { P[K] = 0.0; });
+        static_for<0, SZ>([&](auto K) { P[K] = Real(0); });
         P[ix(0, 0)] = b00;
-        static_for<1, n>([&](auto I) { P[ix(0, I)] = 1.0; });
-        double kap = 1.0;
+        static_for<1, n>([&](auto I) { P[ix(0, I)] = Real(1); });
+        Real kap = Real(1);
         for (int j = m - 1; j >= 1; --j) {
-            kap *= c_dbl[j + 1];
+            kap *= Num<Real>::num(j + 1);
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
                 static_for<i + 1, n>([&](auto K) {
@@ -140,12 +140,12 @@ struct Tpc {
                     P[ix(i, k)] = fma(-al[i - 1], P[ix(i, k)], P[ix(0, k)]);
                 });
             });
-            double t00 = be2[0] * P[ix(0, 1)];
+            Real t00 = be2[0] * P[ix(0, 1)];
             static_for<2, n>([&](auto L) {
                 constexpr int l = L;
                 t00 = fma(be2[l - 1], P[ix(0, l)], t00);
             });
-            const double x00 = kap + P[ix(0, 0)];
+            const Real x00 = kap + P[ix(0, 0)];
             static_for<1, n>([&](auto K) {
                 constexpr int k = K;
                 P[ix(0, k)] = fma(-al[k - 1], P[ix(0, k)], x00);
@@ -154,8 +154,8 @@ struct Tpc {
         }
         {
             // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!
-            const double inv = c_ifact[m];
-            double bs[N];
+            const Real inv = Num<Real>::ifact(m);
+            Real bs[N];
             static_for<0, N>([&](auto I) { bs[I] = be[I] * inv; });
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
@@ -171,24 +171,24 @@ struct Tpc {
             constexpr int i = I;
             static_for<i + 1, n>([&](auto K) {
                 constexpr int k = K;
-                P[ix(i, k)] = clamp_below(P[ix(i, k)], 0.0);
+                P[ix(i, k)] = clamp_below(P[ix(i, k)], Real(0));
             });
         });
         conserve(P, w, iw);
 
         // s squarings: O <- offdiag(X X), X = O + diag(1 + d) >= 0 entrywise, X symmetric
         for (int it = min(defer, s); it < s; ++it) {
-            double X[SZ];
+            Real X[SZ];
             static_for<0, SZ>([&](auto K) { X[K] = P[K]; });
             static_for<0, n>([&](auto I) {
                 constexpr int i = I;
-                X[ix(i, i)] = 1.0 + P[ix(i, i)];
+                X[ix(i, i)] = Real(1) + P[ix(i, i)];
             });
             static_for<0, n>([&](auto I) {
                 constexpr int i = I;
                 static_for<i + 1, n>([&](auto K) {
                     constexpr int k = K;
-                    double acc = X[sx(i, 0)] * X[sx(0, k)];
+                    Real acc = X[sx(i, 0)] * X[sx(0, k)];
                     static_for<1, n>([&](auto L) {
                         constexpr int l = L;
                         acc = fma(X[sx(i, l)], X[sx(l, k)], acc);

@@ -91,6 +91,33 @@ def test_table_b1_constants_in_the_kernels():
     assert [q * r for q, r in qr] == ms and [q + r - 2 for q, r in qr] == list(range(1, 10))
 
 
+def test_single_precision_thresholds_of_eq_b8():
+    """Eq. B.8 names u = 2^-24 as an alternative unit round-off.  The single-precision thresholds compiled
+    into the kernels (dg_params.cuh c_theta32) are recomputed here from Eq. B.4-B.8 with the same 60-digit routine as
+    the u = 2^-53 column above: each constant must satisfy the bound and be tight to 1e-6 (they are floats)."""
+    from mpmath import mp, mpf, factorial, log
+    mp.dps = 60
+    src = open(os.path.join(ROOT, "paper_2509_25347_b200", "csrc", "dg_params.cuh")).read()
+    th = [float(np.float32(x.strip().rstrip("f"))) for x in
+          re.search(r"c_theta32\[kRows\]\s*=\s*\{([^}]*)\}", src, flags=re.S).group(1).split(",")]
+    ms = [2, 4, 6, 9, 12, 16, 20, 25, 30]
+    assert len(th) == 9
+    u = mpf(2) ** -24
+    for m, theta_c in zip(ms, th):
+        c = {}
+        for tot in range(m + 1, m + 140):
+            c[tot] = -sum((mpf(-1) ** (tot - j) / factorial(tot - j)) / factorial(j) for j in range(m + 1, tot + 1))
+        f = lambda t: sum(abs(v) * t ** k for k, v in c.items())
+        bound = lambda t: -log(1 - f(t)) / t
+        t = mpf(theta_c)
+        assert f(t) < 1 and bound(t) <= u
+        assert bound(t * (1 + mpf(10) ** -6)) > u
+    assert all(a < b for a, b in zip(th, th[1:]))
+    # every single-precision threshold is larger than its double-precision twin: fewer squarings for the same norm
+    th64 = [float(x) for x in re.search(r"c_theta\[kRows\]\s*=\s*\{([^}]*)\}", src, flags=re.S).group(1).split(",")]
+    assert all(a > b for a, b in zip(th, th64))
+
+
 def test_workload_generators_are_seeded_and_shaped():
     from paper_2509_25347_b200 import workloads as W
     for cfg, N in [(1, 1), (2, 4), (3, 8), (4, 16), (5, 12)]:
