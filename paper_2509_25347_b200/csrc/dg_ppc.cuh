@@ -23,14 +23,16 @@
 //         Z: {z, 2a+r}                                        (gas, own)
 //     Role 1's pairs are role 0's rotated by one position; together they are all pairs exactly once (for odd g the
 //     antipodal class is computed by both and stored by role 0).
-//   * The matrix is stored by circle DIAGONALS: pair {p, p+d} at table[p][d], d = 0..g, plus row C = a copy of row 0,
-//     plus zv[p] = X[z][p] (zv[C] = zv[0]) and zz = X[z][z].  Rotating every index by one position then moves every
-//     address by the same constant (one table row), so role 1 runs role 0's code on a base pointer shifted by one row:
-//     all shared-memory offsets in the hot loop are immediates.
+//   * The matrix is stored by circle DIAGONALS: pair {p, p+d} at table[p][d], d = 0..g, with X[z][p], w[p] and 1/w[p]
+//     in three more columns of row p, plus row C = a copy of row 0, plus X[z][z] once per role.  Rotating every index
+//     by one position then moves every address by the same constant (one table row), so role 1 runs role 0's code on
+//     a base pointer shifted by one row: no select and no predicate in the hot loop.
+//   * The squaring loops over the rows l of X (two per iteration, operands double-buffered) with the row's operand
+//     offsets in a constant-memory table (LDCU.128 + LDS [R + UR]): 2 KB of loop instead of 29 KB of unrolled code.
 //
-// Measured on B200 (throw-away microbenchmark, N = 16): 3830 cycles per squaring of 16 cells per SM sub-partition,
-// fp64 pipe 69 % busy, shared-memory wavefronts 83 % of peak, 24.4 TFLOP/s of useful flops in the squaring phase;
-// the same mapping with packed storage and role selects (FSEL) reached 57 % / 19.5.
+// Measured on B200 (N = 16, ncu, profiles/): in the squaring loop the fp64 pipe and the shared-memory pipe are
+// co-limiting (17 eight-byte loads per lane per 68 FMAs = one wavefront per 4 FMAs of the SM, exactly the ratio of the
+// two peaks); whole kernel: fp64 pipe ~62 % busy, shared-memory wavefronts ~73 % of peak.
 #pragma once
 #include "dg_params.cuh"
 #include "dg_tpc.cuh"  // static_for, Idx
