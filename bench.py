@@ -168,10 +168,20 @@ def barrier():
         dist.barrier()
 
 
+VARIANT = 0   # --variant: forces a thread mapping (dg_drag_update_variant) for mapping-against-mapping measurements
+
+
+def _update(dg, wl, p_out):
+    if VARIANT == 0:
+        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+    else:
+        dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=VARIANT)
+
+
 def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None):
     """Returns (total ms over `steps` launches, list of per-launch ms)."""
     for _ in range(warmup):
-        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+        _update(dg, wl, p_out)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     barrier()
     torch.cuda.synchronize()
@@ -179,7 +189,7 @@ def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None):
         sampler.start()
     ev[0].record()
     for k in range(steps):
-        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)
+        _update(dg, wl, p_out)
         ev[k + 1].record()
     torch.cuda.synchronize()
     if sampler is not None:
@@ -381,7 +391,7 @@ def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
     p_out = torch.empty_like(wl.p_in)
     total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
     dense_flops, products = algorithmic_flops(wl)
-    _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out)  # untimed: per-cell (m, s)
+    _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=VARIANT)  # untimed: per-cell (m, s)
     flops = useful_flops(wl.N, s, m)
     ms_launch = sum(per) / len(per)
     roof = roofline_for(wl, ms_launch, dense_flops, flops, peaks, hbm_gbs, hbm_src)
@@ -407,6 +417,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[config-1]; 5 = sweep point (give --N)")
     ap.add_argument("--N", type=int, default=None)
+    ap.add_argument("--variant", type=int, default=0, help="force a mapping: 1 thread/cell, 2 warp/cell DMMA, 4 pair/cell")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -416,6 +427,8 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
+    global VARIANT
+    VARIANT = args.variant
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
