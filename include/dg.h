@@ -32,15 +32,18 @@
  * Reproducibility.  For a fixed build and GPU the same call (same pointers' cell ranges, same ncells) gives the same
  * bits, run to run.  A cell's VALUE never depends on other cells beyond rounding: every cell agrees with the exact
  * result to the documented tolerance whatever its neighbours hold.  Its BITS may: the kernels pick the Taylor degree m
- * (any Table B.1 row is admissible for any cell) once per group of cells that share a warp, so computing the same
- * cell as part of a different sub-range of the arrays (another offset or ncells) may change its result at O(u).
+ * (any Table B.1 row is admissible for any cell) once per group of cells that share a warp — 32 cells of similar
+ * stiffness out of a tile of 128 or 256 consecutive cells (tiles start at multiples of their size from cell 0) — so
+ * computing the same cell as part of a different sub-range of the arrays (an offset that is not a multiple of 2048
+ * cells, or another ncells where that cuts a tile short) may change its result at O(u).
  * dg_drag_update_host cuts its chunks so that it stays bit-identical to one dg_drag_update over all cells.
  *
  * Errors.  Every entry point returns a dg_status; nothing throws or aborts across the ABI:
  *     DG_ENULL   a required pointer is NULL (checked only when ncells > 0)
  *     DG_ERANGE  N outside [1, DG_NMAX] or ncells < 0
  *     DG_EALIGN  a pointer is not 8-byte aligned (fp64 arrays; 4-byte for the int32 arrays).  8 bytes is all that is
- *                required; 16-byte aligned base pointers with an even ncells let some kernels move two cells per copy
+ *                required; 16-byte aligned base pointers with an even ncells let the kernels move whole rows of a tile
+ *                per bulk copy (or two cells per copy) instead of one cell per copy — same results, faster
  *     DG_EINVAL  dt negative or not finite, or another scalar argument outside its documented range
  *     DG_ECUDA   the CUDA runtime reported an error (cudaGetLastError after the launch, or a failed copy/alloc);
  *                dg_last_cuda_error() returns its text
@@ -138,10 +141,11 @@ dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float
 /* Same as dg_drag_update_ex with the thread mapping forced (for measuring the mappings against each other; both
  * compute the same arithmetic and agree to rounding):
  *   DG_VARIANT_DEFAULT  the library's measured choice for this N (what dg_drag_update uses)
- *   DG_VARIANT_TPC      thread-per-cell: one thread owns a cell, packed symmetric matrices in registers
+ *   DG_VARIANT_TPC      thread-per-cell: one thread owns a cell, packed symmetric matrices in registers; a warp takes
+ *                       32 consecutive cells
  *   DG_VARIANT_WPC      warp-per-cell: one warp owns a cell, fp64 tensor-core (DMMA) tiles for the squarings
  *   DG_VARIANT_PPC      pair-per-cell: two lanes own a cell, the iterate in a shared-memory tile, cells sorted by
- *                       stiffness inside tiles of 2048 cells before they are handed to the warps
+ *                       stiffness inside tiles of 128 cells before they are handed to the warps (default, N >= 13)
  *   DG_VARIANT_PAPER    NOT the same arithmetic: the paper's own scheme as printed — one thread per cell, dense
  *                       (N+1)x(N+1) fp64 matrices, Table B.1 row minimising Pi_m + s on ||A||_1 (Eq. B.11), Taylor
  *                       polynomial by Algorithm 7, plain squarings (Alg. 6).  A measured reference for the design
@@ -151,6 +155,9 @@ dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float
  *   DG_VARIANT_PAPER_BOUND  as DG_VARIANT_PAPER_ALG2 plus the "second modification": the bound b_exp by Algorithm 8
  *                       and the evaluation with bound test by Algorithm 9; m_out then
  *                       reports the degree actually evaluated, m - q * (blocks the test dropped)
+ *   DG_VARIANT_TPS      thread-per-cell over sorted tiles (default for N <= 12; DG_EINVAL above): a block stages a tile
+ *                       of 128 or 256 consecutive cells in shared memory with bulk copies, counting-sorts it by
+ *                       stiffness and hands its warps chunks of 32 cells that need about the same number of squarings
  * Any other value is DG_EINVAL. */
 #define DG_VARIANT_DEFAULT 0
 #define DG_VARIANT_TPC 1
@@ -159,6 +166,7 @@ dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float
 #define DG_VARIANT_PPC 4
 #define DG_VARIANT_PAPER_ALG2 5
 #define DG_VARIANT_PAPER_BOUND 6
+#define DG_VARIANT_TPS 7
 dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                  const double* p_in, int N, long long ncells, double* p_out, int* s_out, int* m_out,
                                  int variant, void* stream);

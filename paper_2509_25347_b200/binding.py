@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libdg.so")
 DG_NMAX = 16
 DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
 (DG_VARIANT_DEFAULT, DG_VARIANT_TPC, DG_VARIANT_WPC, DG_VARIANT_PAPER, DG_VARIANT_PPC, DG_VARIANT_PAPER_ALG2,
- DG_VARIANT_PAPER_BOUND) = range(7)
+ DG_VARIANT_PAPER_BOUND, DG_VARIANT_TPS) = range(8)
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
            "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy", "dg_drag_update_f32",

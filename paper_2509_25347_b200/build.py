@@ -21,6 +21,7 @@ OBJDIR = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libdg.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 NMAX = 16
+TPS_NMAX = 12  # dg_internal.h kTpsMaxN
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -42,6 +43,8 @@ def _units():
         units.append((f"dg_wpc_kernels_N{n}.o", "dg_wpc_kernels.cu", [f"-DDG_N={n}"]))
         units.append((f"dg_paper_kernels_N{n}.o", "dg_paper_kernels.cu", [f"-DDG_N={n}"]))
         units.append((f"dg_f32_kernels_N{n}.o", "dg_f32_kernels.cu", [f"-DDG_N={n}"]))
+    for n in range(1, TPS_NMAX + 1):
+        units.append((f"dg_tps_kernels_N{n}.o", "dg_tps_kernels.cu", [f"-DDG_N={n}"]))
     for np_ in range(2, NMAX + 1, 2):
         units.append((f"dg_ppc_kernels_NP{np_}.o", "dg_ppc_kernels.cu", [f"-DDG_NP={np_}"]))
     return units

@@ -38,13 +38,21 @@ static const PpcLaunchers* const kPpcTable[DG_NMAX + 1] = {
     &ppc_launchers_NP8,  &ppc_launchers_NP8,  &ppc_launchers_NP10, &ppc_launchers_NP10, &ppc_launchers_NP12, &ppc_launchers_NP12,
     &ppc_launchers_NP14, &ppc_launchers_NP14, &ppc_launchers_NP16, &ppc_launchers_NP16};
 
-// The mapping dg_drag_update uses for each N, chosen from measurements on B200: the thread-per-cell
-// kernel keeps the packed symmetric matrices of one cell in registers up to N = 9 and spills mildly up to N = 12, where
-// it still wins; from N = 13 its spills take over and the pair-per-cell kernel (two lanes per cell, the iterate in a
-// shared-memory tile) wins (2^22 stiff cells, ms: N = 12: 7.0 thread / 7.9 pair; N = 13: 16.2 / 11.2; N = 16: - / 14.8,
-// warp-per-cell DMMA 23.1).
+static const TpsLaunchers* const kTpsTable[DG_NMAX + 1] = {
+    nullptr,           &tps_launchers_N1,  &tps_launchers_N2,  &tps_launchers_N3, &tps_launchers_N4,
+    &tps_launchers_N5, &tps_launchers_N6,  &tps_launchers_N7,  &tps_launchers_N8, &tps_launchers_N9,
+    &tps_launchers_N10, &tps_launchers_N11, &tps_launchers_N12, nullptr,           nullptr,
+    nullptr,           nullptr};
+
+// The mapping dg_drag_update uses for each N, chosen from measurements on B200.  One thread per cell
+// with the packed symmetric matrices in its registers up to N = 12 (mild spills from N = 10), run over stiffness-sorted
+// shared-memory tiles (dg_tps_kernels.cu): 3-25 % faster than the same core over 32 consecutive cells (dg_kernels.cu,
+// kept as DG_VARIANT_TPC) on every workload of BASELINE.json.  From N = 13 the thread-per-cell spills take over and the
+// pair-per-cell kernel (two lanes per cell, the iterate in a shared-memory tile) wins (2^22 stiff cells, ms: N = 12:
+// 5.7 sorted thread / 7.9 pair; N = 13: 16.2 thread / 10.8 pair; N = 16: 13.9 pair, warp-per-cell DMMA 23.1).
 constexpr int kFirstPpcN = 13;
-static inline int default_variant(int N) { return N >= kFirstPpcN ? DG_VARIANT_PPC : DG_VARIANT_TPC; }
+static_assert(kFirstPpcN == kTpsMaxN + 1, "every N has a default kernel");
+static inline int default_variant(int N) { return N >= kFirstPpcN ? DG_VARIANT_PPC : DG_VARIANT_TPS; }
 // The staged dg_expm_scale_square has no pair-per-cell form (it writes dense matrices to HBM: a test path); it keeps the
 // warp-per-cell DMMA kernel from N = 14 and the thread-per-cell one below.
 static inline int expm_variant(int N) { return N >= 14 ? DG_VARIANT_WPC : DG_VARIANT_TPC; }
@@ -73,6 +81,7 @@ cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t 
     if (variant == DG_VARIANT_PAPER_ALG2) return kPaperTable[N]->update[1](a, st);
     if (variant == DG_VARIANT_PAPER_BOUND) return kPaperTable[N]->update[2](a, st);
     if (variant == DG_VARIANT_PPC) return kPpcTable[N]->update(a, N, st);
+    if (variant == DG_VARIANT_TPS) return kTpsTable[N]->update(a, st);
     return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
 }
 
@@ -139,7 +148,8 @@ dg_status dg_drag_update_variant(const double* rho_g, const double* rho_d, const
     dg_status st = check_common(N, ncells, &noop);
     if (st != DG_OK) return st;
     if (!(dt >= 0.0) || !std::isfinite(dt)) return DG_EINVAL;
-    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_PAPER_BOUND) return DG_EINVAL;
+    if (variant < DG_VARIANT_DEFAULT || variant > DG_VARIANT_TPS) return DG_EINVAL;
+    if (variant == DG_VARIANT_TPS && N > kTpsMaxN) return DG_EINVAL;
     if (noop) return DG_OK;
     DG_CHECK_PTR(rho_g);
     DG_CHECK_PTR(rho_d);
@@ -224,7 +234,7 @@ int dg_launches_per_update(int N, long long ncells) {
 
 const char* dg_variant_name(int N) {
     if (N < 1 || N > DG_NMAX) return "";
-    return default_variant(N) == DG_VARIANT_PPC ? kPpcTable[N]->variant : kTable[N]->variant;
+    return default_variant(N) == DG_VARIANT_PPC ? kPpcTable[N]->variant : kTpsTable[N]->variant;
 }
 
 const char* dg_status_string(dg_status st) {

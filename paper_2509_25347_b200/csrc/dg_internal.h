@@ -80,6 +80,17 @@ struct PpcLaunchers {
 extern const PpcLaunchers ppc_launchers_NP2, ppc_launchers_NP4, ppc_launchers_NP6, ppc_launchers_NP8, ppc_launchers_NP10,
     ppc_launchers_NP12, ppc_launchers_NP14, ppc_launchers_NP16;
 
+// Thread-per-cell kernel over stiffness-sorted shared-memory tiles (dg_tps_kernels.cu, one translation unit per N <= 12).
+struct TpsLaunchers {
+    cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    int tile;  // cells per sorted tile: launches over sub-ranges that start on a multiple of it give the same bits
+    const char* variant;
+};
+constexpr int kTpsMaxN = 12;
+extern const TpsLaunchers tps_launchers_N1, tps_launchers_N2, tps_launchers_N3, tps_launchers_N4, tps_launchers_N5,
+    tps_launchers_N6, tps_launchers_N7, tps_launchers_N8, tps_launchers_N9, tps_launchers_N10, tps_launchers_N11,
+    tps_launchers_N12;
+
 // Single-precision thread-per-cell kernel (dg_f32_kernels.cu, one translation unit per N).
 struct F32Launchers {
     cudaError_t (*update)(const UpdateArgsF32&, cudaStream_t);

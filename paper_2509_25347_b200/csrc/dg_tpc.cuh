@@ -131,7 +131,7 @@ struct Tpc {
         P[ix(0, 0)] = b00;
         static_for<1, n>([&](auto I) { P[ix(0, I)] = Real(1); });
         Real kap = Real(1);
-        for (int j = m - 1; j >= 1; --j) {
+        auto horner_step = [&](int j) {
             kap *= Num<Real>::num(j + 1);
             static_for<1, n>([&](auto I) {
                 constexpr int i = I;
@@ -151,6 +151,17 @@ struct Tpc {
                 P[ix(0, k)] = fma(-al[k - 1], P[ix(0, k)], x00);
             });
             P[ix(0, 0)] = fma(b00, x00, t00);
+        };
+        {
+            int j = m - 1;
+            // two steps per trip where the loop overhead is a large part of a step (N = 2..4, measured: 1-2 %)
+            if constexpr (N >= 2 && N <= 4) {
+                for (; j >= 2; j -= 2) {
+                    horner_step(j);
+                    horner_step(j - 1);
+                }
+            }
+            for (; j >= 1; --j) horner_step(j);
         }
         {
             // P_0k = beta_k v_k / m!,  P_ik = beta_i beta_k U_ik / m!

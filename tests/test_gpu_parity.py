@@ -77,12 +77,21 @@ def test_sweep_every_species_count(dg, oracle, cuda, N):
     run_and_compare(dg, oracle, wl)
 
 
-@pytest.mark.parametrize("variant", [1, 2, 4])
+@pytest.mark.parametrize("variant", [1, 2, 4, 7])
 @pytest.mark.parametrize("N", list(range(1, 17)))
 def test_both_thread_mappings_for_every_species_count(dg, oracle, cuda, N, variant):
-    """dg_drag_update_variant: thread-per-cell (1), warp-per-cell DMMA (2) and pair-per-cell (4) each against the
-    oracle, for every N, on the stiff configs[4] generator and on the Dustywave-like configs[2] recipe."""
+    """dg_drag_update_variant: thread-per-cell (1), warp-per-cell DMMA (2), pair-per-cell (4) and thread-per-cell over
+    sorted tiles (7, N <= 12) each against the oracle, for every N, on the stiff configs[4] generator and on the
+    Dustywave-like configs[2] recipe."""
+    if variant == 7 and N > 12:
+        wl = W.make_workload(5, ncells=64, N=N, device=cuda)
+        with pytest.raises(RuntimeError, match="DG_EINVAL"):
+            dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=variant)
+        return
     wl = W.make_workload(5, ncells=700 + 13 * N, N=N, device=cuda)
+    run_and_compare(dg, oracle, wl, variant=variant)
+    # an even cell count with 16-byte aligned rows: whole tiles travel by bulk copies, the ragged last one by 8-byte copies
+    wl = W.make_workload(5, ncells=1024 + 2 * (17 + N), N=N, device=cuda)
     run_and_compare(dg, oracle, wl, variant=variant)
     wl = W.make_workload(3, ncells=333, N=N, device=cuda)
     run_and_compare(dg, oracle, wl, variant=variant)
@@ -330,14 +339,14 @@ def test_extreme_stiffness_and_weak_coupling(dg, oracle, cuda, N):
 def test_extreme_stiffness_against_mpmath(dg, cuda, N):
     """The stiffest cells (dt/t_s = 1e10, ~40 squarings) against mpmath.expm at 90 digits applied to Eq. 17
      retyped here: an arbitrary-precision reference that is neither the oracle nor the CUDA path.
-    N = 8 and 16 run every thread mapping: the default one, thread-per-cell (for N = 8 with the last squaring replaced
-    by a second apply) and the warp-per-cell DMMA kernel, whose diagonal is re-derived from conservation on every other
+    N = 8 and 16 run every thread mapping: the default one (sorted tiles / pair-per-cell), thread-per-cell (for N = 8
+    with the last squaring replaced by a second apply) and the warp-per-cell DMMA kernel, whose diagonal is re-derived from conservation on every other
     squaring only (Eq. 23-24; Theorem 1)."""
     import mpmath as mpm
     from mpmath import mp, mpf
     mp.dps = 90
     wl = _extreme_workload(N, cuda)
-    variants = (0,) if N < 8 else (0, 1, 2, 4)
+    variants = (0, 1) if N < 8 else (0, 1, 2, 4, 7) if N <= 12 else (0, 1, 2, 4)
     outs = {v: dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=v) for v in variants}
     rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(wl.ncells))
     n = N + 1
@@ -360,12 +369,14 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
                     assert abs(mpf(float(o[comp, k])) - refs[comp][k]) <= PARITY_TOL * scale, (N, c, v, comp, k)
 
 
-@pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0), (16, 4), (7, 4)])
+@pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0), (16, 4), (7, 4),
+                                       (1, 7), (2, 0), (8, 7), (12, 0)])
 @pytest.mark.parametrize("ncells", [512, 515, 2050])
 def test_pointers_that_are_8_but_not_16_byte_aligned(dg, oracle, cuda, N, variant, ncells):
     """include/dg.h asks for 8-byte alignment only.  Every array is a view starting one double into its allocation
     (8 mod 16), with even and odd cell counts: the kernels that move two cells per 16-byte copy must fall back to
-    8-byte accesses instead of faulting, and the results must still match the oracle."""
+    8-byte accesses instead of faulting (the sorted-tile kernel: per-thread copies instead of bulk copies, whose rows must
+    be 16-byte aligned), and the results must still match the oracle."""
     wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
 
     def shifted(t):
@@ -422,8 +433,48 @@ def test_pair_per_cell_scheduler_with_wildly_uneven_tiles(dg, oracle, cuda, N):
     assert torch.equal(again, out)               # deterministic whatever the order in which the warps claimed chunks
 
 
+@pytest.mark.parametrize("N", [1, 2, 5, 8, 12])
+def test_sorted_tiles_group_cells_by_stiffness(dg, oracle, cuda, N):
+    """The sorted-tile kernel (DG_VARIANT_TPS, the default for N <= 12) counting-sorts each tile by the exponent of the
+    norm bound and runs chunks of 32 sorted cells per warp.  Cells of very different stiffness interleaved cell by cell
+    (s = 0 next to s ~ 30): every cell must still come back in ITS place, match the oracle where it can referee and
+    conserve momentum; each cell's reported (m, s) must satisfy Theorem 1's premise for its own norm; the call is
+    deterministic; a sub-range that starts on a tile boundary gives the same bits as the whole range (include/dg.h)."""
+    ncells = 256 * 9 + 2 * 51
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
+    c = torch.arange(ncells, device=cuda)
+    wl.t_s[:, c % 3 == 0] = 1e7          # norm ~ 1e-9
+    wl.t_s[:, c % 7 == 1] = 1e-10        # norm ~ 1e8
+    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    torch.cuda.synchronize()
+    assert int(s.max()) >= 25 and int(s.min()) == 0 and int(m.min()) <= 4
+    rho_g, rho_d, t_s, p_in = wl.cells(torch.arange(ncells))
+    got = out.cpu().numpy()
+    assert np.isfinite(got).all()
+    assert float(oracle.conservation_error(got, p_in).max()) <= CONS_TOL
+    norm1 = 2.0 * np.maximum((rho_d / rho_g * wl.dt / t_s).sum(axis=0), (wl.dt / t_s).max(axis=0))
+    ok = norm1 <= 1e6
+    ref = oracle.drag_update(rho_g[ok], rho_d[:, ok], t_s[:, ok], wl.dt, p_in[:, :, ok])
+    assert float(oracle.parity_error(got[:, :, ok], ref, p_in[:, :, ok]).max()) <= PARITY_TOL
+    # Theorem 1's premise with the kernels' closed-form bound on ||S||_2 (DESIGN.md R5), every cell
+    theta = {2: 2.5809568e-8, 4: 3.3971688e-4, 6: 9.0656564e-3, 9: 8.9577602e-2, 12: 2.9961589e-1, 16: 7.8028743e-1,
+             20: 1.4382526, 25: 2.4285825, 30: 3.5396663}
+    bound = (wl.dt / t_s).max(axis=0) + (rho_d / rho_g * wl.dt / t_s).sum(axis=0)
+    sv = s.cpu().numpy(); mv = m.cpu().numpy()
+    th = np.array([theta[int(k)] for k in mv])
+    assert (bound / 2.0 ** sv <= th * (1 + 1e-9)).all()
+    # the cheap cells are not dragged along by the stiff ones of their tile: they run (almost) no squarings
+    assert float(sv[np.asarray(((c % 3 == 0) & (c % 7 != 1)).cpu())].mean()) <= 1.0
+    again = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    assert torch.equal(again, out)
+    off = 2048
+    sub = dg.dg_drag_update(wl.rho_g[off:], wl.rho_d[:, off:].contiguous(), wl.t_s[:, off:].contiguous(), wl.dt,
+                            wl.p_in[:, :, off:].contiguous())
+    assert torch.equal(sub, out[:, :, off:])
+
+
 @pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
-@pytest.mark.parametrize("variant", [0, 1, 2, 4])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4])   # 0 = sorted tiles for N <= 12, pair-per-cell above
 def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
     """include/dg.h: non-finite input gives non-finite output in that cell only.  With the thread-per-cell mapping
     the poisoned cell shares a warp (and the warp's Taylor degree, R8) with 31 healthy ones: they must still
@@ -450,7 +501,8 @@ def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
     assert not bool(torch.isfinite(out[1, :, 41]).all()) and bool(torch.isfinite(out[0, :, 41]).all())
 
 
-@pytest.mark.parametrize("N,ncells", [(1, 33), (4, 127), (8, 1001), (13, 130), (16, 1027), (16, 3)])
+@pytest.mark.parametrize("N,ncells", [(1, 33), (4, 127), (8, 1001), (13, 130), (16, 1027), (16, 3), (2, 512), (8, 1026),
+                                      (12, 256)])
 def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
     """compute-sanitizer is not available on the GPU pool, so out-of-bounds writes are caught with canaries: p_out is
     a window of a larger allocation whose borders must come back untouched, for every kernel that writes momenta."""
@@ -458,7 +510,9 @@ def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
     n = N + 1
     guard = 4096
     size = 3 * n * ncells
-    for which in ("tpc", "wpc", "ppc", "paper", "rk1", "steps"):
+    for which in ("tpc", "wpc", "ppc", "paper", "rk1", "steps", "tps"):
+        if which == "tps" and N > 12:
+            continue
         big = torch.full((size + 2 * guard,), -7.25, dtype=torch.float64, device=cuda)
         p_out = big[guard:guard + size].view(3, n, ncells)
         if which == "rk1":
@@ -466,7 +520,7 @@ def test_no_write_outside_the_output_buffer(dg, cuda, N, ncells):
         elif which == "steps":
             dg.dg_drag_update_steps(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, 3, p_out=p_out)
         else:
-            variant = {"tpc": 1, "wpc": 2, "paper": 3, "ppc": 4}[which]
+            variant = {"tpc": 1, "wpc": 2, "paper": 3, "ppc": 4, "tps": 7}[which]
             dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=variant)
         torch.cuda.synchronize()
         assert bool((big[:guard] == -7.25).all()) and bool((big[guard + size:] == -7.25).all()), which
