@@ -178,8 +178,11 @@ def _update(dg, wl, p_out):
         dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=VARIANT)
 
 
-def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None):
-    """Returns (total ms over `steps` launches, list of per-launch ms)."""
+def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None, per_launch_events=True):
+    """Returns (total ms over `steps` launches, list of per-launch ms).  The total is always one pair of CUDA events around
+    the `steps` launches.  With per_launch_events an event is also recorded after every launch (per-launch minimum); an
+    event between two launches costs the stream a few microseconds, which matters for the ~0.1 ms kernels of the sweep:
+    those are timed without, and `per` is then the average repeated."""
     for _ in range(warmup):
         _update(dg, wl, p_out)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
@@ -190,13 +193,18 @@ def time_device_steps(dg, wl, p_out, steps, warmup, sampler=None):
     ev[0].record()
     for k in range(steps):
         _update(dg, wl, p_out)
-        ev[k + 1].record()
+        if per_launch_events or k == steps - 1:
+            ev[k + 1].record()
     torch.cuda.synchronize()
     if sampler is not None:
         sampler.stop()
     barrier()
-    per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
-    return ev[0].elapsed_time(ev[steps]), per
+    total = ev[0].elapsed_time(ev[steps])
+    if per_launch_events:
+        per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+    else:
+        per = [total / steps] * steps
+    return total, per
 
 
 def measure_peaks(dg, device, sm_count, sm_max_mhz):
@@ -394,21 +402,30 @@ def bench_paper_variant(dg, wl, p_out, steps=2, warmup=1):
     return res
 
 
-def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None):
+def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None, min_region_ms=0.0):
+    """One workload, device-timed.  min_region_ms > 0 (the sweep entries): the number of timed launches is raised (up to
+    400) until the timed region lasts about that long, and no event is recorded between launches — a 0.1 ms kernel timed
+    over five launches with an event after each reads 5-8 % slow (launch latency after the synchronize, event gaps)."""
     p_out = torch.empty_like(wl.p_in)
-    total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler)
+    fine = True
+    if min_region_ms > 0.0:
+        t_est, _ = time_device_steps(dg, wl, p_out, 3, warmup, None, per_launch_events=False)
+        want = int(math.ceil(min_region_ms / max(t_est / 3, 1e-3)))
+        if want > steps:
+            steps, fine = min(want, 400), False
+    total_ms, per = time_device_steps(dg, wl, p_out, steps, warmup, sampler, per_launch_events=fine)
     dense_flops, products = algorithmic_flops(wl)
     _, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, p_out=p_out, variant=VARIANT)  # untimed: per-cell (m, s)
     flops = useful_flops(wl.N, s, m)
     ms_launch = sum(per) / len(per)
     roof = roofline_for(wl, ms_launch, dense_flops, flops, peaks, hbm_gbs, hbm_src)
     res = {"workload": wl.name, "N": wl.N, "ncells": wl.ncells, "ms_per_step": total_ms / steps,
-           "ms_per_launch_min": min(per), "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
+           "ms_per_launch_min": min(per), "timed_launches": steps, "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
            "useful_flops_per_cell": flops / wl.ncells, "dense_flops_per_cell": dense_flops / wl.ncells,
            "dense_products_per_cell": products, "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N),
            "mean_s": float(s.double().mean().item()), "mean_m": float(m.double().mean().item()),
            "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
-    res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs)
+    res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs, steps=5 if fine else max(5, steps))   # same timed-region rule
     res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
     res["paper_as_printed"] = bench_paper_variant(dg, wl, p_out)
     res["paper_as_printed"]["speedup_of_product_path"] = res["paper_as_printed"]["ms_per_launch"] / ms_launch
@@ -495,7 +512,7 @@ def main():
         points = [(c, None) for c in (2, 3, 4) if c != args.config] + [(5, N) for N in W.SWEEP_N]
         for cfg, N in points:
             w2 = W.make_workload(cfg, N=N, device=device)
-            r2, _ = bench_one(dg, w2, max(3, min(args.steps, 5)), 3, peaks, hbm_gbs, hbm_src)
+            r2, _ = bench_one(dg, w2, max(3, min(args.steps, 5)), 3, peaks, hbm_gbs, hbm_src, min_region_ms=20.0)
             sweep.append(r2)
             del w2
             torch.cuda.empty_cache()

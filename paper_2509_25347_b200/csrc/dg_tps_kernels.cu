@@ -39,8 +39,13 @@ constexpr int kWarps = kThreads / 32;
 // Tile size and resident blocks per SM, measured on B200 (2^22 stiff cells): 128-thread blocks with ONE
 // tile each beat larger blocks, larger tiles at fewer blocks per SM and blocks that walk several tiles with the next
 // tile's copies under way: what hides a block's load / sort / store phases is the other blocks on the SM.
-constexpr int kTile = N <= 1 ? 128 : N <= 8 ? 256 : 128;
-constexpr int kMinBlocks = N <= 1 ? 16 : N <= 2 ? 7 : N <= 4 ? 4 : N <= 6 ? 3 : 2;
+#if defined(DG_TPS_TILE) && defined(DG_TPS_MINBLOCKS)  // tuning experiments only
+constexpr int kTile = DG_TPS_TILE;
+constexpr int kMinBlocks = DG_TPS_MINBLOCKS;
+#else
+constexpr int kTile = N <= 1 ? 128 : N <= 10 ? 256 : 128;  // (N = 11, 12: two 256-cell tiles do not fit one SM)
+constexpr int kMinBlocks = N <= 1 ? 16 : N <= 2 ? 7 : N <= 4 ? 4 : N <= 7 ? 3 : 2;
+#endif
 static_assert(kTile % kThreads == 0 && kTile <= 2048 && 2048 % kTile == 0, "tile: whole rounds of the block; divides 2048");
 constexpr int kPerThread = kTile / kThreads;
 constexpr int kSegs = kTile / 32;
@@ -183,10 +188,10 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         unsigned* z = reinterpret_cast<unsigned*>(&sm.seg[0][0]);
         for (int i = t; i < kSegs * kKeys / 2; i += kThreads) z[i] = 0u;
     }
-    // (every warp polls the mbarrier itself: with warp 0 alone polling and the others asleep at the block barrier the
-    // N = 1 kernel measured 5 % slower — the barrier release comes a poll period late)
+    // (only warp 0 polls the mbarrier; the others sleep at the block barrier instead of spending issue slots on the poll:
+    // 1 % at N = 1, where the kernel is issue-bound)
     if (bulk) {
-        mbar_wait(&sm.mbar[0], 0);
+        if (warp == 0) mbar_wait(&sm.mbar[0], 0);
     } else {
         cp_async_wait<1>();
     }
@@ -247,9 +252,12 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         const int pos = sm.base[key[j]] + sm.seg[j * kWarps + warp][key[j]] + rank[j];
         sm.order[pos] = (unsigned short)idx;
     }
-    if (!bulk) cp_async_wait<0>();
-    __syncthreads();  // permutation (and, on the per-thread path, the momenta) visible
-    if (bulk) mbar_wait(&sm.mbar[1], 0);
+    if (bulk) {
+        if (warp == 0) mbar_wait(&sm.mbar[1], 0);
+    } else {
+        cp_async_wait<0>();
+    }
+    __syncthreads();  // permutation and momenta visible
 
     // ---- 3. chunks of 32 sorted cells ------------------------------------------------------------------------------
     // Chunks are dealt to the warps in serpentine order (0 1 2 3 | 3 2 1 0 | ..): the tile is sorted stiffest first, so

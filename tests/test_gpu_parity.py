@@ -615,7 +615,7 @@ def test_single_precision_update(dg, oracle, cuda, N):
 
 
 # ------------------------------------------------------------------ host-buffer end-to-end entry point
-@pytest.mark.parametrize("N,ncells,chunk", [(1, 5000, 0), (4, 10007, 4096), (8, 3001, 1000), (16, 1237, 500)])
+@pytest.mark.parametrize("N,ncells,chunk", [(1, 5000, 0), (4, 10007, 4096), (8, 3001, 1000), (16, 1237, 500), (2, 20480, 2048)])
 def test_host_entry_point_matches_device_entry_point(dg, cuda, N, ncells, chunk):
     wl = W.make_workload(5, ncells=ncells, N=N, device="cpu")
     pin = lambda t: t.pin_memory()
@@ -627,6 +627,15 @@ def test_host_entry_point_matches_device_entry_point(dg, cuda, N, ncells, chunk)
     p = wl.p_in.clone()
     dg.dg_drag_update_host(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p, p_out=p, chunk_cells=chunk)
     assert torch.equal(p, out_h)
+    # rows wider than a 2-D copy's pitch limit (ncells >= 2^28 in real life) go one 1-D copy per row: forced here by
+    # lowering the limit through the environment
+    import os
+    os.environ["DG_HOST_MAX_PITCH"] = "1024"
+    try:
+        out_rows = dg.dg_drag_update_host(h[0], h[1], h[2], wl.dt, h[3], chunk_cells=chunk)
+    finally:
+        del os.environ["DG_HOST_MAX_PITCH"]
+    assert torch.equal(out_rows, out_h)
     dg.dg_host_release()
 
 
