@@ -56,6 +56,15 @@ def test_argument_validation_without_a_gpu(dg):
     assert lib.dg_drag_update_host(p, p, p, 0.1, p, 4, 0, p, 0, -1) == dg.DG_OK
     assert lib.dg_drag_update_host(p, p, p, 0.1, p, 4, 8, None, 0, -1) == dg.DG_ENULL
     assert lib.dg_drag_update_host(p, p, p, 0.1, p, 4, 8, p, -5, -1) == dg.DG_EINVAL
+    # dg_drag_update_variant: unknown variants, and the sorted-tile kernel beyond the species counts it is built for
+    v = lib.dg_drag_update_variant
+    assert v(p, p, p, 0.1, p, 4, 4, p, None, None, 8, None) == dg.DG_EINVAL
+    assert v(p, p, p, 0.1, p, 4, 4, p, None, None, -1, None) == dg.DG_EINVAL
+    assert v(p, p, p, 0.1, p, 13, 4, p, None, None, dg.DG_VARIANT_TPS, None) == dg.DG_EINVAL
+    assert v(p, p, p, 0.1, p, 12, 0, p, None, None, dg.DG_VARIANT_TPS, None) == dg.DG_OK          # ncells = 0: no-op
+    for N in range(1, 17):   # the default mapping named for every N: sorted tiles up to 12, pair per cell above
+        name = dg.dg_variant_name(N)
+        assert ("thread-per-cell" in name) == (N <= 12) and ("pair-per-cell" in name) == (N >= 13), (N, name)
     for st in range(6):
         assert dg.raw().dg_status_string(st).decode().startswith("DG_")
     with pytest.raises(TypeError):
