@@ -13,7 +13,7 @@
 //      address arithmetic or LDGSTS, whole 128-byte lines whatever the order the cells are processed in;
 //   2. each thread forms the sort key of its cells (conflict-free column reads), a stable counting sort over 64 keys
 //      (MATCH.ANY ranks inside a warp, per-segment counters, one warp scans them) writes the permutation;
-//   3. warps claim chunks of 32 sorted cells from a counter; a lane reads ITS cell's column of the tile (permuted
+//   3. the warps take chunks of 32 sorted cells in serpentine order; a lane reads ITS cell's column of the tile (permuted
 //      shared-memory reads), runs a1..a4 in registers, applies the result to the cell's momenta in place in the tile;
 //   4. the 3n momentum rows leave shared -> global with one bulk copy per row.
 // One tile per block, several blocks per SM: the copies of one block overlap the arithmetic of the others.
