@@ -473,6 +473,36 @@ def test_sorted_tiles_group_cells_by_stiffness(dg, oracle, cuda, N):
     assert torch.equal(sub, out[:, :, off:])
 
 
+def test_sorted_tiles_against_consecutive_cells_on_random_sizes(dg, cuda):
+    """The two thread-per-cell mappings share their arithmetic core but group the cells differently (and move them
+    differently: bulk copies / per-thread copies / ragged tails).  120 seeded random (N, ncells, recipe) triples around
+    the tile and warp boundaries: the results agree to rounding, momentum is conserved, the default entry point gives the
+    same bits as the forced variant, and in place gives the same bits as out of place."""
+    import random
+    rnd = random.Random(7)
+    sizes = [1, 2, 31, 32, 33, 127, 128, 129, 255, 256, 257, 511, 512, 513, 1000, 1024, 2047, 2048, 2050]
+    for it in range(120):
+        N = rnd.randint(1, 12)
+        nc = rnd.choice(sizes + [rnd.randint(1, 9000), 4096 + rnd.randint(0, 600)])
+        wl = W.make_workload(rnd.choice([5, 2, 3]), ncells=nc, N=N, device=cuda)
+        if rnd.random() < 0.3:
+            c = torch.arange(nc, device=cuda)
+            wl.t_s[:, c % 5 == 1] = 1e-9
+            wl.t_s[:, c % 3 == 0] = 1e6
+        o1 = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=dg.DG_VARIANT_TPC)[0]
+        o7 = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, variant=dg.DG_VARIANT_TPS)[0]
+        o0 = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+        p = wl.p_in.clone()
+        dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p, p_out=p)
+        torch.cuda.synchronize()
+        scale = wl.p_in.abs().amax(dim=(0, 1))
+        err = float(((o1 - o7).abs().amax(dim=(0, 1)) / scale).max())
+        cons = float(((o7.sum(1) - wl.p_in.sum(1)).abs() / wl.p_in.abs().sum(1)).max())
+        assert bool(torch.isfinite(o7).all()), (N, nc)
+        assert err <= 2e-13 and cons <= CONS_TOL, (N, nc, err, cons)
+        assert torch.equal(o0, o7) and torch.equal(p, o7), (N, nc)
+
+
 @pytest.mark.parametrize("N", [1, 4, 8, 13, 16])
 @pytest.mark.parametrize("variant", [0, 1, 2, 4])   # 0 = sorted tiles for N <= 12, pair-per-cell above
 def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
