@@ -357,6 +357,51 @@ def bench_rk1(dg, wl, p_out, hbm_gbs, steps=5, warmup=3):
             "hbm_frac": gbs / hbm_gbs}
 
 
+def _timed_ms(f, steps, warmup):
+    for _ in range(warmup):
+        f()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        f()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def bench_energy(dg, wl, p_out, ms_update, hbm_gbs, steps=5, warmup=2):
+    """dg_drag_update_energy (Eq. 4, R20): the fused update between two O(N) kernels
+    that read the densities and the momenta before / after it.  Algorithmic bytes per cell: the update's 8(8N+7) plus
+    8(2(1 + N + 3n) + 3) for the two energy kernels (rho_g, rho_d, p, and E read / written)."""
+    E_in = torch.ones(wl.ncells, dtype=torch.float64, device=wl.rho_g.device)
+    E_out = torch.empty_like(E_in)
+    ms = _timed_ms(lambda: dg.dg_drag_update_energy(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, E_in, 0.5, p_out=p_out,
+                                                    E_out=E_out), steps, warmup)
+    n = wl.N + 1
+    extra = 8 * (2 * (1 + wl.N + 3 * n) + 3)
+    gbs_extra = extra * wl.ncells / (max(ms - ms_update, 1e-6) * 1e-3) / 1e9
+    return {"ms_per_launch_sequence": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "over_plain_update": ms / ms_update,
+            "extra_bytes_per_cell": extra, "energy_kernels_gbs": gbs_extra, "energy_kernels_hbm_frac": gbs_extra / hbm_gbs}
+
+
+def bench_f32(dg, wl, ms_update, fp32_peak_tflops, steps=5, warmup=2):
+    """dg_drag_update_f32 (Eq. B.8 with u = 2^-24) on the same fields rounded to float: useful flops
+    of ITS (m, s) against the fp32 FMA peak (128 lanes per SM), and the time against the fp64 path."""
+    f = lambda t: t.to(torch.float32).contiguous()
+    rho_g, rho_d, t_s, p_in = f(wl.rho_g), f(wl.rho_d), f(wl.t_s), f(wl.p_in)
+    out = torch.empty_like(p_in)
+    _, s, m = dg.dg_drag_update_f32(rho_g, rho_d, t_s, wl.dt, p_in, p_out=out)
+    ms = _timed_ms(lambda: dg.dg_drag_update_f32(rho_g, rho_d, t_s, wl.dt, p_in, p_out=out), steps, warmup)
+    flops = useful_flops(wl.N, s, m)
+    peak = fp32_peak_tflops
+    tf = flops / (ms * 1e-3) / 1e12
+    hbm = 4 * (8 * wl.N + 7) * wl.ncells / (ms * 1e-3) / 1e9
+    return {"ms_per_launch": ms, "cells_per_s": wl.ncells / (ms * 1e-3), "achieved_tflops": tf, "fp32_peak_tflops": peak,
+            "alu_frac": tf / peak, "achieved_gbs": hbm, "mean_s": float(s.double().mean().item()),
+            "mean_m": float(m.double().mean().item()), "fp64_over_f32_time": ms_update / ms}
+
+
 def bench_paper_variant(dg, wl, p_out, steps=2, warmup=1):
     """The paper's own scheme as printed (one thread per cell, dense matrices, Alg. 7 + plain squarings; SURVEY.md
     §8(f) rank 3) on the same buffers, for the design comparison on the same hardware: with the row chosen by
@@ -427,6 +472,9 @@ def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None, min_
            "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
     res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs, steps=5 if fine else max(5, steps))   # same timed-region rule
     res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
+    if wl.ncells <= (1 << 22):   # the two rank-4 entry points, on the 2^21..2^22-cell workloads (they need extra buffers)
+        res["energy"] = bench_energy(dg, wl, p_out, ms_launch, hbm_gbs)
+        res["f32"] = bench_f32(dg, wl, ms_launch, 2.0 * peaks["fp64_nominal_tflops"])   # 128 fp32 vs 64 fp64 FMA lanes per SM
     res["paper_as_printed"] = bench_paper_variant(dg, wl, p_out)
     res["paper_as_printed"]["speedup_of_product_path"] = res["paper_as_printed"]["ms_per_launch"] / ms_launch
     del p_out
