@@ -5,9 +5,12 @@
 // drag terms of Eq. 4 integrate exactly: the work term is the change of the gas kinetic energy, the heating term is
 // w times the kinetic energy the drag dissipates (dK/dt = -sum_i rho_d,i |v_d,i - v_g|^2 / T_s,i by Eq. 3, 6), so
 //     E_g(t+dt) = E_g(t) + [KE_g(t+dt) - KE_g(t)] + w [K(t) - K(t+dt)],    K = |M_g|^2/(2 rho_g) + sum_i |M_d,i|^2/(2 rho_d,i).
-// Three launches on the caller's stream: k_energy_pre (the terms at t, from p_in — before the update, so that p_out may
-// alias p_in), the fused drag update (dg_drag_update's kernel for this N), k_energy_post (the terms at t+dt, from p_out).
-// Both energy kernels are one thread per cell, every field row read coalesced: O(N) flops, HBM-bound.
+// N <= 12: ONE launch — the sorted-tile kernel (dg_tps_kernels.cu) holds rho_g, rho_d, p_in and p_out of a tile in shared
+// memory anyway and forms the two kinetic-energy sums on the way (one more tile row for E).
+// N >= 13: three launches on the caller's stream: k_energy_pre (the terms at t, from p_in — before the update, so that
+// p_out may alias p_in), the fused drag update (dg_drag_update's kernel for this N), k_energy_post (the terms at t+dt,
+// from p_out).  Both energy kernels are one thread per cell, every field row read coalesced: O(N) flops, HBM-bound;
+// they add 7-12 % to a 10-14 ms update.
 #include <cmath>
 #include <cstdint>
 
@@ -17,6 +20,8 @@
 namespace dg {
 dg_status cuda_status(cudaError_t e);
 cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t st);
+bool has_fused_energy(int N);
+cudaError_t launch_update_energy(int N, const UpdateArgs& a, const double* E_in, double* E_out, double w, cudaStream_t st);
 
 namespace {
 constexpr int kThreads = 256;
@@ -80,6 +85,10 @@ extern "C" dg_status dg_drag_update_energy(const double* rho_g, const double* rh
         if (reinterpret_cast<uintptr_t>(p) & 7u) return DG_EALIGN;
     }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (has_fused_energy(N)) {  // N <= 12: one launch, the sums are formed inside the sorted-tile kernel
+        UpdateArgs a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, nullptr, nullptr};
+        return cuda_status(launch_update_energy(N, a, E_in, E_out, w, st));
+    }
     const unsigned grid = (unsigned)((ncells + kThreads - 1) / kThreads);
     k_energy_pre<<<grid, kThreads, 0, st>>>(rho_g, rho_d, p_in, E_in, w, N, ncells, E_out);
     cudaError_t e = cudaGetLastError();

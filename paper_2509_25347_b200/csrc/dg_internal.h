@@ -83,6 +83,8 @@ extern const PpcLaunchers ppc_launchers_NP2, ppc_launchers_NP4, ppc_launchers_NP
 // Thread-per-cell kernel over stiffness-sorted shared-memory tiles (dg_tps_kernels.cu, one translation unit per N <= 12).
 struct TpsLaunchers {
     cudaError_t (*update)(const UpdateArgs&, cudaStream_t);
+    // dg_drag_update_energy in ONE launch: the update plus E_out = E_in + [KE_g] + w [K(t) - K(t+dt)] (s_out / m_out unused)
+    cudaError_t (*update_energy)(const UpdateArgs&, const double* E_in, double* E_out, double w, cudaStream_t);
     int tile;  // cells per sorted tile: launches over sub-ranges that start on a multiple of it give the same bits
     const char* variant;
 };

@@ -17,6 +17,9 @@
 //      shared-memory reads), runs a1..a4 in registers, applies the result to the cell's momenta in place in the tile;
 //   4. the 3n momentum rows leave shared -> global with one bulk copy per row.
 // One tile per block, several blocks per SM: the copies of one block overlap the arithmetic of the others.
+// The same kernel, instantiated with kEnergy, is dg_drag_update_energy for N <= 12: the tile already holds rho_g, rho_d,
+// p_in and p_out, so the kinetic energies before and after the update (Eq. 4, R20) cost one more row (E) and a few
+// FMAs per species instead of two further passes over the momenta in HBM.
 // Unaligned pointers (8 but not 16 bytes), odd row strides and the ragged last tile take per-thread 8-byte copies.
 #include <cstdint>
 
@@ -54,15 +57,23 @@ constexpr int kRowsIn = 1 + 2 * N;  // rho_g, rho_d[N], t_s[N]
 constexpr int kRowsP = 3 * n;       // p[3][n]
 constexpr unsigned kFull = 0xffffffffu;
 
-struct Smem {
+template <bool kEnergy>
+struct SmemT {
     double F[kRowsIn][kTile];             // fields of the tile
     double PM[kRowsP][kTile];             // momenta of the tile: p_in, overwritten in place by p_out
+    double EN[kEnergy ? kTile : 2];       // (energy variant) gas energy of the tile: E_in, overwritten in place by E_out
     unsigned long long mbar[2];           // [0] fields landed, [1] momenta landed
     unsigned short seg[kSegs][kKeys];     // counting sort: per 32-cell segment and key, count -> offset inside the key
     unsigned short base[kKeys];           // first sorted position of each key
     unsigned short order[kTile];          // sorted position -> cell of the tile
 };
-constexpr size_t kSmemBytes = sizeof(Smem);
+struct EnergyArgs {  // dg_drag_update_energy: E_in, E_out [ncells], heating fraction w
+    const double* E_in;
+    double* E_out;
+    double w;
+};
+template <bool kEnergy>
+constexpr size_t kSmemBytesT = sizeof(SmemT<kEnergy>);
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
@@ -115,9 +126,10 @@ __device__ __forceinline__ int sort_key(double norm) {
     return min(max(e, 1), kKeys - 1);
 }
 
-__global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs g, int bulk_ok) {
+template <bool kEnergy>
+__global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs g, EnergyArgs eg, int bulk_ok) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+    SmemT<kEnergy>& sm = *reinterpret_cast<SmemT<kEnergy>*>(smem_raw);
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const long long nc = g.ncells;
     const long long tile_base = (long long)blockIdx.x * kTile;
@@ -137,7 +149,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         __syncthreads();
         if (warp == 0) {
             if (lane == 0) {
-                mbar_expect_tx(&sm.mbar[0], kRowsIn * kRowBytes);
+                mbar_expect_tx(&sm.mbar[0], (kRowsIn + (kEnergy ? 1 : 0)) * kRowBytes);
                 mbar_expect_tx(&sm.mbar[1], kRowsP * kRowBytes);
             }
             __syncwarp();
@@ -147,6 +159,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
                                     tile_base;
                 bulk_g2s(F[r], src, kRowBytes, &sm.mbar[0]);
             }
+            if (kEnergy && lane == 31) bulk_g2s(sm.EN, eg.E_in + tile_base, kRowBytes, &sm.mbar[0]);
             for (int r = lane; r < kRowsP; r += 32)
                 bulk_g2s(PM[r], g.p_in + (long long)r * nc + tile_base, kRowBytes, &sm.mbar[1]);
         }
@@ -157,6 +170,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
             if (idx < count) {
                 const long long c = tile_base + idx;
                 cp_async8(&F[0][idx], g.rho_g + c);
+                if constexpr (kEnergy) cp_async8(&sm.EN[idx], eg.E_in + c);
                 const double* pd = g.rho_d + c;
                 const double* pt = g.t_s + c;
 #pragma unroll
@@ -283,10 +297,16 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
                 a[i] = F[1 + N + i][cell];
-                sym_weights(F[1 + i][cell] * irg, w[i], iw[i]);
+                const double rd = F[1 + i][cell];
+                sym_weights(rd * irg, w[i], iw[i]);
                 if (!valid) {
                     a[i] = 0.0;
                     w[i] = iw[i] = 1.0;
+                }
+                if constexpr (kEnergy) {
+                    // 1 / (2 rho_d,i) replaces rho_d,i in the cell's column of the tile (a species with rho_d = 0 carries
+                    // no energy); true division: one per species and cell, off the critical path
+                    if (valid) F[1 + i][cell] = rd > 0.0 ? 0.5 / rd : 0.0;
                 }
             });
         }
@@ -305,11 +325,18 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         }
         if (valid) {
             const int napply = 1 << min(Core::kDefer, s);
+            // (energy variant) sums over the components of |M_g|^2 and of sum_i |M_d,i|^2 / (2 rho_d,i), before and after
+            double g2_in = 0.0, kd_in = 0.0, g2_out = 0.0, kd_out = 0.0;
+            auto kinetic = [&](const double (&pv)[n], double& g2, double& kd) {
+                g2 = fma(pv[0], pv[0], g2);
+                static_for<1, n>([&](auto K) { kd = fma(pv[K] * pv[K], F[K][cell], kd); });
+            };
 #pragma unroll 1
             for (int comp = 0; comp < 3; ++comp) {
                 double* pc = &PM[comp * n][cell];
                 double p[n], q[n];
                 static_for<0, n>([&](auto K) { p[K] = pc[K * kTile]; });
+                if constexpr (kEnergy) kinetic(p, g2_in, kd_in);
                 auto apply_once = [&]() {
                     static_for<0, n>([&](auto K) {
                         constexpr int kq = K;
@@ -330,6 +357,14 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
 #pragma unroll 1
                 for (int rep = 0; rep < napply; ++rep) apply_once();
                 static_for<0, n>([&](auto K) { pc[K * kTile] = p[K]; });
+                if constexpr (kEnergy) kinetic(p, g2_out, kd_out);
+            }
+            if constexpr (kEnergy) {
+                // E_g(t+dt) = E_g(t) + [KE_g(t+dt) - KE_g(t)] + w [K(t) - K(t+dt)],  K = KE_g + sum_i |M_d,i|^2 / (2 rho_d,i)
+                const double h = 0.5 * F[0][cell];  // 1 / (2 rho_g)
+                const double keg_in = g2_in * h, keg_out = g2_out * h;
+                const double k_in = keg_in + kd_in, k_out = keg_out + kd_out;
+                sm.EN[cell] = sm.EN[cell] + ((keg_out - keg_in) + eg.w * (k_in - k_out));
             }
         }
     }
@@ -340,6 +375,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         __syncthreads();
         if (warp == 0) {
             for (int r = lane; r < kRowsP; r += 32) bulk_s2g(g.p_out + (long long)r * nc + tile_base, PM[r], kRowBytes);
+            if (kEnergy && lane == 31) bulk_s2g(eg.E_out + tile_base, sm.EN, kRowBytes);
             asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
             asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory");  // the tile must outlive the reads
         }
@@ -355,38 +391,46 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
                     *po = PM[r][idx];
                     po += nc;
                 }
+                if constexpr (kEnergy) eg.E_out[tile_base + idx] = sm.EN[idx];
             }
         }
     }
 }
 
-cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
+template <bool kEnergy>
+cudaError_t launch(const UpdateArgs& a, const EnergyArgs& eg, cudaStream_t st) {
     static bool configured[64] = {false};
+    constexpr size_t smem = kSmemBytesT<kEnergy>;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
     if (!configured[dev]) {
-        e = cudaFuncSetAttribute(k_update_tps, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        e = cudaFuncSetAttribute(k_update_tps<kEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured[dev] = true;
     }
     const long long ntiles = (a.ncells + kTile - 1) / kTile;
     if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;
     // bulk copies need 16-byte aligned rows: 16-byte aligned base pointers and an even row stride
-    const uintptr_t bits = reinterpret_cast<uintptr_t>(a.rho_g) | reinterpret_cast<uintptr_t>(a.rho_d) |
-                           reinterpret_cast<uintptr_t>(a.t_s) | reinterpret_cast<uintptr_t>(a.p_in) |
-                           reinterpret_cast<uintptr_t>(a.p_out);
+    uintptr_t bits = reinterpret_cast<uintptr_t>(a.rho_g) | reinterpret_cast<uintptr_t>(a.rho_d) |
+                     reinterpret_cast<uintptr_t>(a.t_s) | reinterpret_cast<uintptr_t>(a.p_in) |
+                     reinterpret_cast<uintptr_t>(a.p_out);
+    if (kEnergy) bits |= reinterpret_cast<uintptr_t>(eg.E_in) | reinterpret_cast<uintptr_t>(eg.E_out);
     const int bulk_ok = ((bits & 15u) == 0 && (a.ncells & 1) == 0) ? 1 : 0;
-    k_update_tps<<<(unsigned)ntiles, kThreads, kSmemBytes, st>>>(a, bulk_ok);
+    k_update_tps<kEnergy><<<(unsigned)ntiles, kThreads, smem, st>>>(a, eg, bulk_ok);
     return cudaGetLastError();
+}
+cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) { return launch<false>(a, EnergyArgs{nullptr, nullptr, 0.0}, st); }
+cudaError_t launch_update_energy(const UpdateArgs& a, const double* E_in, double* E_out, double w, cudaStream_t st) {
+    return launch<true>(a, EnergyArgs{E_in, E_out, w}, st);
 }
 
 }  // namespace
 
 #define DG_CAT_(a, b) a##b
 #define DG_CAT(a, b) DG_CAT_(a, b)
-extern const TpsLaunchers DG_CAT(tps_launchers_N, DG_N) = {launch_update, kTile,
+extern const TpsLaunchers DG_CAT(tps_launchers_N, DG_N) = {launch_update, launch_update_energy, kTile,
                                                            "thread-per-cell over stiffness-sorted shared-memory tiles"};
 
 }  // namespace dg

@@ -84,12 +84,15 @@ def test_heating_n1_closed_form(oracle):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("N", [1, 2, 4, 8, 13, 16])
-def test_gpu_energy_update_matches_the_oracle(dg, oracle, cuda, N):
+@pytest.mark.parametrize("ncells", [1501, 2048, 2570])
+@pytest.mark.parametrize("N", [1, 2, 4, 7, 8, 12, 13, 16])
+def test_gpu_energy_update_matches_the_oracle(dg, oracle, cuda, N, ncells):
     """dg_drag_update_energy through the C ABI against the oracle: momenta at BASELINE.json's tolerance, gas energy to
-    1e-13 of the cell's energy scale (E_g and the kinetic energies: a handful of fp64 products and one difference)."""
+    1e-13 of the cell's energy scale (E_g and the kinetic energies: a handful of fp64 products and one difference).
+    N <= 12 is one launch of the sorted-tile kernel (whole tiles by bulk copies for the even cell counts, per-thread copies
+    for the odd one and the ragged tails), N >= 13 three launches."""
     from paper_2509_25347_b200 import workloads as W
-    wl = W.make_workload(5, ncells=1500 + N, N=N, device=cuda)
+    wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
     wl.rho_d[0, ::5] = 0.0
     g = torch.Generator(device="cpu"); g.manual_seed(N)
     E_in = (1.0 + 10 * torch.rand(wl.ncells, generator=g, dtype=torch.float64)).to(cuda)
@@ -104,6 +107,15 @@ def test_gpu_energy_update_matches_the_oracle(dg, oracle, cuda, N):
         kin = kin + np.where(rho_d > 0, (p_in[:, 1:] ** 2).sum(axis=0) / (2 * rd), 0.0).sum(axis=0)
         scale = np.abs(E_in.cpu().numpy()) + kin
         assert float((np.abs(E_out.cpu().numpy().astype(LD) - E_ref) / scale).max()) <= 1e-13
+    # the momenta are those of the plain update, bit for bit
+    assert torch.equal(p_out, dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in))
+    # E arrays that are 8 but not 16 bytes aligned (no bulk copies): same bits
+    big = torch.empty(wl.ncells + 3, dtype=torch.float64, device=cuda)
+    E_sh = big[1:1 + wl.ncells]; E_sh.copy_(E_in)
+    big2 = torch.empty(wl.ncells + 3, dtype=torch.float64, device=cuda)
+    E_sh_out = big2[1:1 + wl.ncells]
+    p3, _ = dg.dg_drag_update_energy(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, E_sh, 0.5, E_out=E_sh_out)
+    assert torch.equal(p3, p_out) and torch.equal(E_sh_out, E_out)
     # in place (p_out aliases p_in, E_out aliases E_in) gives the same bits
     p2 = wl.p_in.clone(); E2 = E_in.clone()
     dg.dg_drag_update_energy(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p2, E2, 0.5, p_out=p2, E_out=E2)
