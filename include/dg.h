@@ -133,7 +133,8 @@ dg_status dg_drag_update_energy(const double* rho_g, const double* rho_d, const 
  * The same path a1..a5 with every array and every operation in fp32, and (m, s) chosen against the scaling thresholds
  * theta_m of Eq. B.4-B.8 recomputed for the unit round-off of IEEE single precision (the paper's Table B.1 is the
  * u = 2^-53 column; Eq. B.8 names 2^-24 as an alternative).  Layouts as above with float elements; pointers 4-byte
- * aligned; p_out may alias p_in; s_out, m_out (int32 [ncells]) nullable.  Agrees with the exact result to about
+ * aligned (16-byte aligned arrays with ncells a multiple of 4 move whole tile rows per bulk copy: same results, faster);
+ * p_out may alias p_in; s_out, m_out (int32 [ncells]) nullable.  Agrees with the exact result to about
  * (s + m + 8)(N + 2) 2^-24 max|p_in| per cell; total momentum to a few 2^-24. */
 dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float* t_s, float dt, const float* p_in,
                              int N, long long ncells, float* p_out, int* s_out, int* m_out, void* stream);

@@ -3,9 +3,9 @@
     python -m paper_2509_25347_b200.build [--force] [--verbose]
 
 One object per translation unit, compiled in parallel: dg_kernels.cu, dg_wpc_kernels.cu, dg_paper_kernels.cu and
-dg_f32_kernels.cu once
-per species count N (-DDG_N=<N>), dg_ppc_kernels.cu once per even number of dust slots (-DDG_NP=<NP>), plus
-dg_api.cu, dg_peaks.cu, dg_host.cu, dg_energy.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
+dg_f32_kernels.cu once per species count N (-DDG_N=<N>), dg_ppc_kernels.cu once per even number of dust slots
+(-DDG_NP=<NP>), dg_tps_kernels.cu once per N <= 12 in double and once in single precision (-DDG_TPS_F32), plus dg_api.cu,
+dg_peaks.cu, dg_host.cu, dg_energy.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
 nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 arithmetic must stay IEEE (the kernels' own Newton
 reciprocals are explicit, dg_params.cuh).  Extra nvcc flags for an experiment can be passed in DG_EXTRA_FLAGS.
 """
@@ -45,6 +45,7 @@ def _units():
         units.append((f"dg_f32_kernels_N{n}.o", "dg_f32_kernels.cu", [f"-DDG_N={n}"]))
     for n in range(1, TPS_NMAX + 1):
         units.append((f"dg_tps_kernels_N{n}.o", "dg_tps_kernels.cu", [f"-DDG_N={n}"]))
+        units.append((f"dg_tps_f32_kernels_N{n}.o", "dg_tps_kernels.cu", [f"-DDG_N={n}", "-DDG_TPS_F32"]))
     for np_ in range(2, NMAX + 1, 2):
         units.append((f"dg_ppc_kernels_NP{np_}.o", "dg_ppc_kernels.cu", [f"-DDG_NP={np_}"]))
     return units

@@ -44,6 +44,12 @@ static const TpsLaunchers* const kTpsTable[DG_NMAX + 1] = {
     &tps_launchers_N10, &tps_launchers_N11, &tps_launchers_N12, nullptr,           nullptr,
     nullptr,           nullptr};
 
+static const TpsF32Launchers* const kTpsF32Table[DG_NMAX + 1] = {
+    nullptr,                &tps_f32_launchers_N1,  &tps_f32_launchers_N2,  &tps_f32_launchers_N3, &tps_f32_launchers_N4,
+    &tps_f32_launchers_N5,  &tps_f32_launchers_N6,  &tps_f32_launchers_N7,  &tps_f32_launchers_N8, &tps_f32_launchers_N9,
+    &tps_f32_launchers_N10, &tps_f32_launchers_N11, &tps_f32_launchers_N12, nullptr,               nullptr,
+    nullptr,                nullptr};
+
 // The mapping dg_drag_update uses for each N, chosen from measurements on B200.  One thread per cell
 // with the packed symmetric matrices in its registers up to N = 12 (mild spills from N = 10), run over stiffness-sorted
 // shared-memory tiles (dg_tps_kernels.cu): 3-25 % faster than the same core over 32 consecutive cells (dg_kernels.cu,
@@ -214,6 +220,8 @@ dg_status dg_drag_update_f32(const float* rho_g, const float* rho_d, const float
     DG_CHECK_OPT_PTR(s_out);
     DG_CHECK_OPT_PTR(m_out);
     UpdateArgsF32 a{rho_g, rho_d, t_s, dt, p_in, ncells, p_out, s_out, m_out};
+    // same choice of mapping as in double precision: sorted tiles up to N = 12, the consecutive-cell kernel above
+    if (N <= kTpsMaxN) return cuda_status(kTpsF32Table[N]->update(a, static_cast<cudaStream_t>(stream)));
     return cuda_status(kF32Table[N]->update(a, static_cast<cudaStream_t>(stream)));
 }
 

@@ -93,6 +93,15 @@ extern const TpsLaunchers tps_launchers_N1, tps_launchers_N2, tps_launchers_N3, 
     tps_launchers_N6, tps_launchers_N7, tps_launchers_N8, tps_launchers_N9, tps_launchers_N10, tps_launchers_N11,
     tps_launchers_N12;
 
+// The sorted-tile kernel in single precision (dg_tps_kernels.cu compiled with -DDG_TPS_F32, one translation unit per N <= 12).
+struct TpsF32Launchers {
+    cudaError_t (*update)(const UpdateArgsF32&, cudaStream_t);
+    int tile;
+};
+extern const TpsF32Launchers tps_f32_launchers_N1, tps_f32_launchers_N2, tps_f32_launchers_N3, tps_f32_launchers_N4,
+    tps_f32_launchers_N5, tps_f32_launchers_N6, tps_f32_launchers_N7, tps_f32_launchers_N8, tps_f32_launchers_N9,
+    tps_f32_launchers_N10, tps_f32_launchers_N11, tps_f32_launchers_N12;
+
 // Single-precision thread-per-cell kernel (dg_f32_kernels.cu, one translation unit per N).
 struct F32Launchers {
     cudaError_t (*update)(const UpdateArgsF32&, cudaStream_t);

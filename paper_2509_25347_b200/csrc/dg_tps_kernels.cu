@@ -35,7 +35,15 @@ namespace {
 
 constexpr int N = DG_N;
 constexpr int n = N + 1;
-using Core = Tpc<N>;
+// -DDG_TPS_F32: the same kernel in single precision (dg_drag_update_f32: float arrays, the u = 2^-24 thresholds of Eq. B.8)
+#ifdef DG_TPS_F32
+using Real = float;
+using Args = UpdateArgsF32;
+#else
+using Real = double;
+using Args = UpdateArgs;
+#endif
+using Core = Tpc<N, Real>;
 constexpr int SZ = Core::SZ;
 constexpr int kThreads = 128;
 constexpr int kWarps = kThreads / 32;
@@ -45,6 +53,9 @@ constexpr int kWarps = kThreads / 32;
 #if defined(DG_TPS_TILE) && defined(DG_TPS_MINBLOCKS)  // tuning experiments only
 constexpr int kTile = DG_TPS_TILE;
 constexpr int kMinBlocks = DG_TPS_MINBLOCKS;
+#elif defined(DG_TPS_F32)  // half the bytes and about half the registers per cell
+constexpr int kTile = N <= 1 ? 128 : 256;
+constexpr int kMinBlocks = N <= 1 ? 16 : N <= 2 ? 14 : N <= 6 ? 6 : N <= 8 ? 4 : 3;
 #else
 constexpr int kTile = N <= 1 ? 128 : N <= 10 ? 256 : 128;  // (N = 11, 12: two 256-cell tiles do not fit one SM)
 constexpr int kMinBlocks = N <= 1 ? 16 : N <= 2 ? 7 : N <= 4 ? 4 : N <= 7 ? 3 : 2;
@@ -59,8 +70,8 @@ constexpr unsigned kFull = 0xffffffffu;
 
 template <bool kEnergy>
 struct SmemT {
-    double F[kRowsIn][kTile];             // fields of the tile
-    double PM[kRowsP][kTile];             // momenta of the tile: p_in, overwritten in place by p_out
+    Real F[kRowsIn][kTile];               // fields of the tile
+    Real PM[kRowsP][kTile];               // momenta of the tile: p_in, overwritten in place by p_out
     double EN[kEnergy ? kTile : 2];       // (energy variant) gas energy of the tile: E_in, overwritten in place by E_out
     unsigned long long mbar[2];           // [0] fields landed, [1] momenta landed
     unsigned short seg[kSegs][kKeys];     // counting sort: per 32-cell segment and key, count -> offset inside the key
@@ -78,6 +89,9 @@ constexpr size_t kSmemBytesT = sizeof(SmemT<kEnergy>);
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async8(float* dst_smem, const float* src_gmem) {  // (one element: 4 bytes)
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int Pending>
@@ -121,13 +135,17 @@ __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, u
 // Sort key of a cell: the binary exponent of the norm bound max_i a_i + sum_i eps_i a_i (R5) mapped to
 // 1..63 (2^-30 .. 2^31, clamped; a non-finite norm gets 63: stiffest).  Key 0 is reserved for the slots past the end of
 // a ragged tile.  Larger key = more squarings; the sort is descending.
+__device__ __forceinline__ int sort_key(float norm) {
+    const int e = (int)(((unsigned)__float_as_int(norm) >> 23) & 0xffu) - 127 + 32;  // NaN / Inf: 0xff -> large
+    return min(max(e, 1), kKeys - 1);
+}
 __device__ __forceinline__ int sort_key(double norm) {
     const int e = (int)(((unsigned)__double2hiint(norm) >> 20) & 0x7ffu) - 1023 + 32;  // NaN / Inf: 0x7ff -> large
     return min(max(e, 1), kKeys - 1);
 }
 
 template <bool kEnergy>
-__global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs g, EnergyArgs eg, int bulk_ok) {
+__global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(Args g, EnergyArgs eg, int bulk_ok) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     SmemT<kEnergy>& sm = *reinterpret_cast<SmemT<kEnergy>*>(smem_raw);
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -136,9 +154,9 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
     const long long left = nc - tile_base;
     const int count = left < kTile ? (int)left : kTile;
     const bool bulk = bulk_ok && count == kTile;  // block-uniform
-    constexpr unsigned kRowBytes = kTile * sizeof(double);
-    double(&F)[kRowsIn][kTile] = sm.F;
-    double(&PM)[kRowsP][kTile] = sm.PM;
+    constexpr unsigned kRowBytes = kTile * sizeof(Real);
+    Real(&F)[kRowsIn][kTile] = sm.F;
+    Real(&PM)[kRowsP][kTile] = sm.PM;
     // ---- 1. the tile's rows: global -> shared ------------------------------------------------------------------
     if (bulk) {
         if (t == 0) {
@@ -154,7 +172,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
             }
             __syncwarp();
             for (int r = lane; r < kRowsIn; r += 32) {
-                const double* src = (r == 0 ? g.rho_g : r <= N ? g.rho_d + (long long)(r - 1) * nc
+                const Real* src = (r == 0 ? g.rho_g : r <= N ? g.rho_d + (long long)(r - 1) * nc
                                                                : g.t_s + (long long)(r - 1 - N) * nc) +
                                     tile_base;
                 bulk_g2s(F[r], src, kRowBytes, &sm.mbar[0]);
@@ -171,8 +189,8 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
                 const long long c = tile_base + idx;
                 cp_async8(&F[0][idx], g.rho_g + c);
                 if constexpr (kEnergy) cp_async8(&sm.EN[idx], eg.E_in + c);
-                const double* pd = g.rho_d + c;
-                const double* pt = g.t_s + c;
+                const Real* pd = g.rho_d + c;
+                const Real* pt = g.t_s + c;
 #pragma unroll
                 for (int i = 0; i < N; ++i) {
                     cp_async8(&F[1 + i][idx], pd);
@@ -187,7 +205,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         for (int j = 0; j < kPerThread; ++j) {
             const int idx = t + j * kThreads;
             if (idx < count) {
-                const double* pp = g.p_in + tile_base + idx;
+                const Real* pp = g.p_in + tile_base + idx;
 #pragma unroll
                 for (int r = 0; r < kRowsP; ++r) {
                     cp_async8(&PM[r][idx], pp);
@@ -219,12 +237,12 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         int kk = 0;
         if (idx < count) {
             // (1 / rho_g and a_i = dt / t_s,i replace rho_g and t_s,i in the tile: step 3 reads them back)
-            const double irg = fast_rcp(F[0][idx]);
+            const Real irg = fast_rcp(F[0][idx]);
             F[0][idx] = irg;
-            double sb = 0.0, amax = 0.0;
+            Real sb = Real(0), amax = Real(0);
 #pragma unroll
             for (int i = 0; i < N; ++i) {
-                const double a = g.dt * fast_rcp(F[1 + N + i][idx]);
+                const Real a = g.dt * fast_rcp(F[1 + N + i][idx]);
                 F[1 + N + i][idx] = a;
                 sb = fma(F[1 + i][idx] * irg, a, sb);
                 amax = fmax(amax, a);
@@ -291,27 +309,27 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         const int cell = sm.order[valid ? pos : j * 32];
 
         // a1: eps_i (Eq. 14), a_i = dt alpha_i (Eq. 15), symmetrising weights; a lane without a cell gets the identity
-        double a[N], w[N], iw[N];
+        Real a[N], w[N], iw[N];
         {
-            const double irg = F[0][cell];
+            const Real irg = F[0][cell];
             static_for<0, N>([&](auto I) {
                 constexpr int i = I;
                 a[i] = F[1 + N + i][cell];
-                const double rd = F[1 + i][cell];
+                const Real rd = F[1 + i][cell];
                 sym_weights(rd * irg, w[i], iw[i]);
                 if (!valid) {
-                    a[i] = 0.0;
-                    w[i] = iw[i] = 1.0;
+                    a[i] = Real(0);
+                    w[i] = iw[i] = Real(1);
                 }
                 if constexpr (kEnergy) {
                     // 1 / (2 rho_d,i) replaces rho_d,i in the cell's column of the tile (a species with rho_d = 0 carries
                     // no energy); true division: one per species and cell, off the critical path
-                    if (valid) F[1 + i][cell] = rd > 0.0 ? 0.5 / rd : 0.0;
+                    if (valid) F[1 + i][cell] = rd > Real(0) ? Real(0.5) / rd : Real(0);
                 }
             });
         }
         // a2-a4
-        double P[SZ];
+        Real P[SZ];
         int m, s;
         Core::template expm<Core::kDefer>(a, w, iw, P, m, s);
         if (valid) {
@@ -327,14 +345,14 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
             const int napply = 1 << min(Core::kDefer, s);
             // (energy variant) sums over the components of |M_g|^2 and of sum_i |M_d,i|^2 / (2 rho_d,i), before and after
             double g2_in = 0.0, kd_in = 0.0, g2_out = 0.0, kd_out = 0.0;
-            auto kinetic = [&](const double (&pv)[n], double& g2, double& kd) {
-                g2 = fma(pv[0], pv[0], g2);
-                static_for<1, n>([&](auto K) { kd = fma(pv[K] * pv[K], F[K][cell], kd); });
+            auto kinetic = [&](const Real (&pv)[n], double& g2, double& kd) {
+                g2 = fma((double)pv[0], (double)pv[0], g2);
+                static_for<1, n>([&](auto K) { kd = fma((double)pv[K] * (double)pv[K], (double)F[K][cell], kd); });
             };
 #pragma unroll 1
             for (int comp = 0; comp < 3; ++comp) {
-                double* pc = &PM[comp * n][cell];
-                double p[n], q[n];
+                Real* pc = &PM[comp * n][cell];
+                Real p[n], q[n];
                 static_for<0, n>([&](auto K) { p[K] = pc[K * kTile]; });
                 if constexpr (kEnergy) kinetic(p, g2_in, kd_in);
                 auto apply_once = [&]() {
@@ -345,7 +363,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
                     });
                     static_for<0, n>([&](auto I) {
                         constexpr int i = I;
-                        double y = 0.0;
+                        Real y = Real(0);
                         static_for<0, n>([&](auto K) {
                             constexpr int kq = K;
                             y = fma(P[Core::sx(i, kq)], q[kq], y);
@@ -385,7 +403,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
         for (int j = 0; j < kPerThread; ++j) {
             const int idx = t + j * kThreads;
             if (idx < count) {
-                double* po = g.p_out + tile_base + idx;
+                Real* po = g.p_out + tile_base + idx;
 #pragma unroll
                 for (int r = 0; r < kRowsP; ++r) {
                     *po = PM[r][idx];
@@ -398,7 +416,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(UpdateArgs 
 }
 
 template <bool kEnergy>
-cudaError_t launch(const UpdateArgs& a, const EnergyArgs& eg, cudaStream_t st) {
+cudaError_t launch(const Args& a, const EnergyArgs& eg, cudaStream_t st) {
     static bool configured[64] = {false};
     constexpr size_t smem = kSmemBytesT<kEnergy>;
     int dev = 0;
@@ -417,20 +435,29 @@ cudaError_t launch(const UpdateArgs& a, const EnergyArgs& eg, cudaStream_t st) {
                      reinterpret_cast<uintptr_t>(a.t_s) | reinterpret_cast<uintptr_t>(a.p_in) |
                      reinterpret_cast<uintptr_t>(a.p_out);
     if (kEnergy) bits |= reinterpret_cast<uintptr_t>(eg.E_in) | reinterpret_cast<uintptr_t>(eg.E_out);
-    const int bulk_ok = ((bits & 15u) == 0 && (a.ncells & 1) == 0) ? 1 : 0;
+    constexpr long long kPer16 = 16 / sizeof(Real);  // elements per 16 bytes: the row stride must be a multiple of it
+    const int bulk_ok = ((bits & 15u) == 0 && a.ncells % kPer16 == 0) ? 1 : 0;
     k_update_tps<kEnergy><<<(unsigned)ntiles, kThreads, smem, st>>>(a, eg, bulk_ok);
     return cudaGetLastError();
 }
+#ifdef DG_TPS_F32
+cudaError_t launch_update(const UpdateArgsF32& a, cudaStream_t st) { return launch<false>(a, EnergyArgs{nullptr, nullptr, 0.0}, st); }
+#else
 cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) { return launch<false>(a, EnergyArgs{nullptr, nullptr, 0.0}, st); }
 cudaError_t launch_update_energy(const UpdateArgs& a, const double* E_in, double* E_out, double w, cudaStream_t st) {
     return launch<true>(a, EnergyArgs{E_in, E_out, w}, st);
 }
+#endif
 
 }  // namespace
 
 #define DG_CAT_(a, b) a##b
 #define DG_CAT(a, b) DG_CAT_(a, b)
+#ifdef DG_TPS_F32
+extern const TpsF32Launchers DG_CAT(tps_f32_launchers_N, DG_N) = {launch_update, kTile};
+#else
 extern const TpsLaunchers DG_CAT(tps_launchers_N, DG_N) = {launch_update, launch_update_energy, kTile,
                                                            "thread-per-cell over stiffness-sorted shared-memory tiles"};
+#endif
 
 }  // namespace dg

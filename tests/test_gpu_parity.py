@@ -596,7 +596,7 @@ def test_equal_velocity_state_is_a_fixed_point(dg, cuda):
 
 
 # ------------------------------------------------------------------ single precision (Eq. B.8 with u = 2^-24)
-@pytest.mark.parametrize("N", [1, 2, 4, 8, 12, 16])
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 6, 8, 12, 13, 16])
 def test_single_precision_update(dg, oracle, cuda, N):
     """dg_drag_update_f32 against the (unchanged, long-double) oracle run on the SAME float inputs widened exactly to
     fp64.  Tolerance, derived in DESIGN.md §10 before the kernel was written: the truncation error is below u32 = 2^-24
@@ -605,7 +605,9 @@ def test_single_precision_update(dg, oracle, cuda, N):
     propagated by stochastic-like matrices); the build (reciprocals, eps, sqrt) adds a few u32:
         per cell  |p_gpu - p_exact| <= (s + m + 8) (N + 2) 2^-24 max|p_in|,    conservation  <= 4 (N + 2) 2^-24 sum|p_in|."""
     u32 = 2.0 ** -24
-    for cfg, ncells in ((5, 3000 + N), (2, 2500), (3, 700)):
+    # (N <= 12 runs the sorted-tile kernel: 3000 + N and 700 exercise its per-thread copies and ragged tiles, 2500 and 4096
+    # — multiples of four floats — its bulk copies)
+    for cfg, ncells in ((5, 3000 + N), (2, 2500), (3, 700), (5, 4096)):
         wl = W.make_workload(cfg, ncells=ncells, N=N, device=cuda)
         f = lambda t: t.to(torch.float32).contiguous()
         rho_g, rho_d, t_s, p_in = f(wl.rho_g), f(wl.rho_d), f(wl.t_s), f(wl.p_in)
@@ -642,6 +644,16 @@ def test_single_precision_update(dg, oracle, cuda, N):
     p = p_in.clone()
     dg.dg_drag_update_f32(rho_g, rho_d, t_s, wl.dt, p, p_out=p)
     assert torch.equal(p, out)
+    # arrays that are 4 but not 16 bytes aligned: same bits as the aligned call
+    def shifted(t):
+        big = torch.empty(t.numel() + 5, dtype=t.dtype, device=t.device)
+        v = big[1:1 + t.numel()].view(t.shape)
+        v.copy_(t)
+        assert v.data_ptr() % 16 == 4
+        return v
+    out_sh = shifted(torch.zeros_like(p_in))
+    dg.dg_drag_update_f32(shifted(rho_g), shifted(rho_d), shifted(t_s), wl.dt, shifted(p_in), p_out=out_sh)
+    assert torch.equal(out_sh, out)
 
 
 # ------------------------------------------------------------------ host-buffer end-to-end entry point
