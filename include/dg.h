@@ -124,7 +124,8 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
  * fraction w (0 = no frictional heating, 1 = all of it) is deposited into the gas.  With w = 1,
  * E_g + sum_i |M_d,i|^2/(2 rho_d,i) is conserved.  A species with rho_d,i = 0 carries no energy.
  * in : rho_g, rho_d, t_s, p_in, E_in [ncells] (device), dt, w.   out: p_out (may alias p_in), E_out [ncells] (may alias
- * E_in).  One launch on `stream` for N <= 12 (the sums are formed inside the update kernel), three for N >= 13.  DG_EINVAL if w is outside [0, 1]; otherwise the errors of dg_drag_update. */
+ * E_in).  One launch on `stream` for N <= 12 (the sums are formed inside the update kernel), three for N >= 13.
+ * DG_EINVAL if w is outside [0, 1]; otherwise the errors of dg_drag_update. */
 dg_status dg_drag_update_energy(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                 const double* p_in, const double* E_in, double w, int N, long long ncells,
                                 double* p_out, double* E_out, void* stream);
