@@ -70,8 +70,8 @@ __device__ __forceinline__ void cp_async_wait_all() {
     asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
 }
 
-// One warp sorts the tile starting at cell `base` (count cells) into order[]: key = binary exponent of the norm bound
-// max_i a_i + sum_i eps_i a_i (R5), stiffest first, non-finite first of all, ties in cell order; entries
+// One warp sorts the tile starting at cell `base` (count cells) into order[]: key = the squarings the norm bound
+// max_i a_i + sum_i eps_i a_i (R5) needs with the m = 30 row (its binary exponent below the last threshold), stiffest first, non-finite first of all, ties in cell order; entries
 // past `count` sort last.  keys: kTile words of scratch in the warp's own tile.  Species-major loads: all the lane's
 // cells for one species are in flight together.
 __device__ __noinline__ void sort_tile_warp(const double* rho_g, const double* rho_d, const double* t_s, double dt,
@@ -109,8 +109,15 @@ __device__ __noinline__ void sort_tile_warp(const double* rho_g, const double* r
 #pragma unroll
     for (int j = 0; j < kPerLane; ++j) {
         const int idx = lane + j * 32;
-        const unsigned e = ((unsigned)__double2hiint(sb[j] + amax[j]) >> 20) & 0x7ffu;  // 0x7ff: Inf / NaN
-        const unsigned key = (idx < count) ? 0x7ffu - e : 0xfffu;
+        // Above the last threshold of Table B.1 the key is the number of squarings the cell needs with the m = 30 row:
+        // s = e - t + [f > g] (dg_params.cuh) changes with the mantissa INSIDE a binade, and sorted by the binary exponent
+        // alone cells of s and s + 1 sit interleaved in every chunk of that binade (4 % more squarings per chunk).  Below
+        // it (s = 0) the key is the binary exponent.  Inf / NaN: largest.  Monotone in the norm; the sort is descending.
+        const double nrm = sb[j] + amax[j];
+        const unsigned e = ((unsigned)__double2hiint(nrm) >> 20) & 0x7ffu;
+        const unsigned v = (nrm > c_theta[kRows - 1]) ? 0x800u + (unsigned)min(scaling_exponent(nrm, c_theta[kRows - 1]), 0x7fe)
+                                                      : (e == 0x7ffu ? 0xfffu : e);
+        const unsigned key = (idx < count) ? 0xfffu - v : 0x1000u;
         mine[j] = (key << 16) | (unsigned)idx;
     }
     const unsigned k0 = __shfl_sync(kFullMask, mine[0], 0) >> 16;
