@@ -23,7 +23,8 @@
  *
  * Ownership.  The library owns no caller-visible memory and keeps no global state that affects results.  All
  * buffers are caller-allocated and caller-freed.  The dg_* device entry points allocate nothing and use no
- * workspace.  dg_drag_update_host keeps a private device staging area that dg_host_release() frees.
+ * workspace.  dg_drag_update_host keeps a private device staging area that dg_host_release() frees;
+ * dg_drag_update_host_static stages in a fixed array inside the library image instead and allocates nothing.
  *
  * Streams and asynchrony.  `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  * entry points only enqueue work and return; they never synchronise.  They are re-entrant and may be called
@@ -47,6 +48,7 @@
  *     DG_EINVAL  dt negative or not finite, or another scalar argument outside its documented range
  *     DG_ECUDA   the CUDA runtime reported an error (cudaGetLastError after the launch, or a failed copy/alloc);
  *                dg_last_cuda_error() returns its text
+ *     DG_ECAPACITY  dg_drag_update_host_static only: ncells exceeds what its fixed staging array holds for this N
  * ncells == 0 is DG_OK and a no-op.
  *
  * Pre-conditions that are NOT checked on the device (PAPER.md is silent; they are what Eq. 14-15 need):
@@ -64,7 +66,10 @@ extern "C" {
 #define DG_NMAX 16
 #define DG_VERSION 100 /* 0.1.0 */
 
-typedef enum { DG_OK = 0, DG_EINVAL = 1, DG_ENULL = 2, DG_EALIGN = 3, DG_ERANGE = 4, DG_ECUDA = 5 } dg_status;
+typedef enum {
+    DG_OK = 0, DG_EINVAL = 1, DG_ENULL = 2, DG_EALIGN = 3, DG_ERANGE = 4, DG_ECUDA = 5,
+    DG_ECAPACITY = 6 /* dg_drag_update_host_static only: the cells do not fit its fixed staging array */
+} dg_status;
 
 /* ---- stage a1: assemble A = dt * Omega  (Eq. 14, 15, 17) ---------------------------------
  * in : rho_g, rho_d, t_s (device), dt.   out: A [n*n][ncells] (device), dense, including the structural zeros.
@@ -185,6 +190,39 @@ dg_status dg_drag_update_host(const double* rho_g, const double* rho_d, const do
                               int device);
 /* Frees the staging area and streams of dg_drag_update_host (all devices).  Safe to call at any time. */
 dg_status dg_host_release(void);
+
+/* ---- the same update on HOST buffers, for callers that cannot allocate device memory ---------------------------
+ * dg_drag_update_host obtains its device staging area with cudaMalloc.  That rules it out for a caller whose own
+ * memory pool has claimed the whole GPU at start-up (the request would fail), for a time-step loop that must not
+ * stall (cudaMalloc / cudaFree synchronise the device), for a process held to a device-memory quota, and for a plug-in
+ * whose host application forbids allocation after initialisation.  This entry point is for them: it makes no
+ * cudaMalloc, cudaFree or any other allocating call, and creates no streams or events.  Its staging area is a fixed
+ * array of DG_STATIC_STAGE_BYTES inside the library image, which every GPU that loads the library's module for this
+ * entry point holds from that moment until the process exits, whether the entry point is called again or not.
+ *
+ * in : rho_g, rho_d, t_s, p_in (HOST, layouts above with row pitch ncells), dt.   out: p_out (HOST), may alias p_in.
+ * Runs on the CURRENT device, entirely on `stream`: four host-to-device copies, the kernel dg_drag_update uses for
+ * this N over all ncells at once, one device-to-host copy; then it waits for `stream`, so p_out is complete on return.
+ * The result is bit-identical to dg_drag_update_host and to dg_drag_update on the same cells.
+ *
+ * Size limit.  A cell needs 8N + 7 doubles of staging (inputs, momenta in, momenta out), so
+ *     ncells <= DG_STATIC_STAGE_BYTES / (8 * (8N + 7))     (279 620 cells at N = 1, 59 074 at N = 8, 31 068 at N = 16).
+ * A larger ncells returns DG_ECAPACITY before any CUDA call is made; nothing is copied and p_out is untouched.  There
+ * is no internal chunking: a caller with more cells compacts them into pieces of at most that many cells and calls once
+ * per piece (pieces that are multiples of 2048 cells reproduce the bits of one launch over everything).
+ *
+ * First call.  The first call on each device resolves the array's device address (cudaGetSymbolAddress), which also
+ * makes the CUDA runtime load the module and place the array on that device.  Make that first call during start-up:
+ * before any stream capture is begun, and at a point where a one-off driver-side set-up cost is acceptable.
+ *
+ * Sharing.  There is ONE array per device, shared by every call in the process, and it keeps the previous call's
+ * bytes.  That is harmless for a single caller — each call overwrites every value its kernel reads, and nothing needs
+ * to start at zero, so nothing is cleared — but two calls whose GPU work can overlap (two host threads, whatever their
+ * streams) race on the array and corrupt each other's results.  The library does not serialise them: the caller must.
+ * Other errors as dg_drag_update_host. */
+#define DG_STATIC_STAGE_BYTES 33554432 /* 32 MiB */
+dg_status dg_drag_update_host_static(const double* rho_g, const double* rho_d, const double* t_s, double dt,
+                                     const double* p_in, int N, long long ncells, double* p_out, void* stream);
 
 /* ---- measurement helpers (used by bench.py; not on the data path) --------------------------------------------
  * dg_peak_kernel enqueues ONE launch of a microbenchmark kernel on `stream` and returns in *work the number of

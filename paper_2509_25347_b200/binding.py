@@ -14,13 +14,14 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libdg.so")
 
 DG_NMAX = 16
-DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA = range(6)
+DG_OK, DG_EINVAL, DG_ENULL, DG_EALIGN, DG_ERANGE, DG_ECUDA, DG_ECAPACITY = range(7)
+DG_STATIC_STAGE_BYTES = 32 << 20
 (DG_VARIANT_DEFAULT, DG_VARIANT_TPC, DG_VARIANT_WPC, DG_VARIANT_PAPER, DG_VARIANT_PPC, DG_VARIANT_PAPER_ALG2,
  DG_VARIANT_PAPER_BOUND, DG_VARIANT_TPS) = range(8)
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
            "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy", "dg_drag_update_f32",
-           "dg_drag_update_host", "dg_host_release", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
+           "dg_drag_update_host", "dg_host_release", "dg_drag_update_host_static", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
            "dg_status_string", "dg_last_cuda_error", "dg_version")
 
 
@@ -51,6 +52,7 @@ def _load():
     lib.dg_drag_update_energy.argtypes = [vp, vp, vp, dbl, vp, vp, dbl, i32, ll, vp, vp, vp]
     lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
     lib.dg_host_release.argtypes = []
+    lib.dg_drag_update_host_static.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
     lib.dg_peak_kernel.argtypes = [i32, i32, vp, ll, C.POINTER(dbl), vp]
     lib.dg_launches_per_update.argtypes = [i32, ll]
     lib.dg_variant_name.argtypes = [i32]
@@ -245,6 +247,24 @@ def dg_drag_update_host(rho_g, rho_d, t_s, dt, p_in, p_out=None, chunk_cells=0, 
 
 def dg_host_release():
     _check(_lib.dg_host_release(), "dg_host_release")
+
+
+def dg_drag_update_host_static(rho_g, rho_d, t_s, dt, p_in, p_out=None):
+    """The fused update on HOST tensors for callers that must not allocate device memory (a host code whose pool owns
+    the whole GPU, a loop that cannot take cudaMalloc's device-wide stall, a fixed memory quota): the library call
+    stages in a fixed 32 MiB array built into libdg.so instead of asking for memory.  At most
+    DG_STATIC_STAGE_BYTES // (8 * (8N + 7)) cells per call, DgError(DG_ECAPACITY) beyond; runs on the current device and
+    torch's current stream and returns when p_out is complete.  Calls share that one array: never let two overlap.
+    (Only the C call is allocation-free; this wrapper still makes the host result tensor when p_out is None.)"""
+    N, ncells = rho_d.shape
+    n = N + 1
+    if p_out is None:
+        p_out = torch.empty_like(p_in)
+    st = _lib.dg_drag_update_host_static(_host(rho_g, "rho_g", (ncells,)), _host(rho_d, "rho_d", (N, ncells)),
+                                         _host(t_s, "t_s", (N, ncells)), float(dt), _host(p_in, "p_in", (3, n, ncells)),
+                                         N, ncells, _host(p_out, "p_out", (3, n, ncells)), _stream())
+    _check(st, "dg_drag_update_host_static")
+    return p_out
 
 
 def dg_peak_kernel(kind, iters, scratch):

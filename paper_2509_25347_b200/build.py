@@ -5,7 +5,7 @@
 One object per translation unit, compiled in parallel: dg_kernels.cu, dg_wpc_kernels.cu, dg_paper_kernels.cu and
 dg_f32_kernels.cu once per species count N (-DDG_N=<N>), dg_ppc_kernels.cu once per even number of dust slots
 (-DDG_NP=<NP>), dg_tps_kernels.cu once per N <= 12 in double and once in single precision (-DDG_TPS_F32), plus dg_api.cu,
-dg_peaks.cu, dg_host.cu, dg_energy.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
+dg_peaks.cu, dg_host.cu, dg_host_static.cu, dg_energy.cu.  Objects are cached under csrc/build/ and rebuilt when a source or header is newer.
 nvcc cross-compiles without a GPU.  Never --use_fast_math: fp64 arithmetic must stay IEEE (the kernels' own Newton
 reciprocals are explicit, dg_params.cuh).  Extra nvcc flags for an experiment can be passed in DG_EXTRA_FLAGS.
 """
@@ -37,7 +37,7 @@ def _nvcc():
 def _units():
     """(object name, source, extra flags)"""
     units = [("dg_api.o", "dg_api.cu", []), ("dg_peaks.o", "dg_peaks.cu", []), ("dg_host.o", "dg_host.cu", []),
-             ("dg_energy.o", "dg_energy.cu", [])]
+             ("dg_energy.o", "dg_energy.cu", []), ("dg_host_static.o", "dg_host_static.cu", [])]
     for n in range(1, NMAX + 1):
         units.append((f"dg_kernels_N{n}.o", "dg_kernels.cu", [f"-DDG_N={n}"]))
         units.append((f"dg_wpc_kernels_N{n}.o", "dg_wpc_kernels.cu", [f"-DDG_N={n}"]))

@@ -259,6 +259,9 @@ const char* dg_status_string(dg_status st) {
         case DG_EALIGN: return "DG_EALIGN: pointer is not 8-byte aligned";
         case DG_ERANGE: return "DG_ERANGE: N outside [1, 16] or ncells < 0";
         case DG_ECUDA: return "DG_ECUDA: CUDA runtime error (see dg_last_cuda_error)";
+        case DG_ECAPACITY:
+            return "DG_ECAPACITY: ncells * 8 * (8N + 7) bytes exceed the fixed 32 MiB staging array of "
+                   "dg_drag_update_host_static (it never allocates; split the cells or use dg_drag_update_host)";
     }
     return "unknown dg_status";
 }
