@@ -190,6 +190,10 @@ dg_status dg_drag_update_host(const double* rho_g, const double* rho_d, const do
                               int device);
 /* Frees the staging area and streams of dg_drag_update_host (all devices).  Safe to call at any time. */
 dg_status dg_host_release(void);
+/* Test hook, not needed in normal use: lowers the largest row pitch (bytes) for which dg_drag_update_host uses one
+ * strided 2-D copy per array; rows with a larger pitch are copied one by one (what happens by itself from
+ * ncells >= 2^28).  0 restores the device's own limit.  Results do not depend on it.  DG_EINVAL if bytes < 0. */
+dg_status dg_host_set_max_pitch(long long bytes);
 
 /* ---- the same update on HOST buffers, for callers that cannot allocate device memory ---------------------------
  * dg_drag_update_host obtains its device staging area with cudaMalloc.  That rules it out for a caller whose own
@@ -233,7 +237,9 @@ dg_status dg_drag_update_host_static(const double* rho_g, const double* rho_d, c
  * iters: loop trip count per thread (kinds 0-2). */
 dg_status dg_peak_kernel(int kind, int iters, double* scratch, long long scratch_bytes, double* work, void* stream);
 
-/* Number of kernels the last device entry point launched for these arguments (the launch plan; 0 if ncells == 0). */
+/* Number of kernels ONE call of dg_drag_update (or _ex, _variant, _f32, _rk1) enqueues for these arguments: 1, or 0
+ * if ncells == 0.  Not for the other entry points: dg_drag_update_steps enqueues nsteps times as many,
+ * dg_drag_update_energy 1 for N <= 12 and 3 above, dg_drag_update_host one per chunk. */
 int dg_launches_per_update(int N, long long ncells);
 /* Human-readable description of the kernel variant dg_drag_update uses for N (static storage). */
 const char* dg_variant_name(int N);

@@ -21,7 +21,7 @@ DG_STATIC_STAGE_BYTES = 32 << 20
 
 EXPORTS = ("dg_drag_matrix_build", "dg_expm_scale_square", "dg_drag_apply", "dg_drag_update", "dg_drag_update_ex",
            "dg_drag_update_variant", "dg_drag_update_steps", "dg_drag_rk1", "dg_drag_update_energy", "dg_drag_update_f32",
-           "dg_drag_update_host", "dg_host_release", "dg_drag_update_host_static", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
+           "dg_drag_update_host", "dg_host_release", "dg_host_set_max_pitch", "dg_drag_update_host_static", "dg_peak_kernel", "dg_launches_per_update", "dg_variant_name",
            "dg_status_string", "dg_last_cuda_error", "dg_version")
 
 
@@ -52,6 +52,7 @@ def _load():
     lib.dg_drag_update_energy.argtypes = [vp, vp, vp, dbl, vp, vp, dbl, i32, ll, vp, vp, vp]
     lib.dg_drag_update_host.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, ll, i32]
     lib.dg_host_release.argtypes = []
+    lib.dg_host_set_max_pitch.argtypes = [ll]
     lib.dg_drag_update_host_static.argtypes = [vp, vp, vp, dbl, vp, i32, ll, vp, vp]
     lib.dg_peak_kernel.argtypes = [i32, i32, vp, ll, C.POINTER(dbl), vp]
     lib.dg_launches_per_update.argtypes = [i32, ll]
@@ -247,6 +248,11 @@ def dg_drag_update_host(rho_g, rho_d, t_s, dt, p_in, p_out=None, chunk_cells=0, 
 
 def dg_host_release():
     _check(_lib.dg_host_release(), "dg_host_release")
+
+
+def dg_host_set_max_pitch(nbytes):
+    """Test hook: rows of dg_drag_update_host whose pitch exceeds `nbytes` are copied one by one (0 = device limit)."""
+    _check(_lib.dg_host_set_max_pitch(int(nbytes)), "dg_host_set_max_pitch")
 
 
 def dg_drag_update_host_static(rho_g, rho_d, t_s, dt, p_in, p_out=None):

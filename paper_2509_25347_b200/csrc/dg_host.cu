@@ -5,9 +5,9 @@
 // with a stream each keep the H2D copy of chunk k+1, the kernel of chunk k and the D2H copy of chunk k-1 in flight
 // together (the GPU has separate copy engines per direction).  No arithmetic here: the kernel is the one
 // dg_drag_update launches.
+#include <atomic>
 #include <cmath>
 #include <cstdint>
-#include <cstdlib>
 #include <mutex>
 
 #include "../../include/dg.h"
@@ -35,6 +35,7 @@ struct Ctx {
     std::mutex mu;         // one caller at a time per device; callers on different devices do not wait for each other
 };
 Ctx g_ctx[kMaxDevices];
+std::atomic<size_t> g_pitch_cap{0};  // dg_host_set_max_pitch: 0 = the device's own limit
 
 #define DG_TRY(x)                           \
     do {                                    \
@@ -67,12 +68,10 @@ cudaError_t ensure(Ctx& c, int device, size_t bytes) {
 // copy per row when the host pitch (ncells * 8 bytes) exceeds what a 2-D copy accepts (2^31 - 1 bytes: ncells >= 2^28).
 cudaError_t copy_rows(const Ctx& c, void* dst, size_t dpitch, const void* src, size_t spitch, size_t width, size_t rows,
                       cudaMemcpyKind kind, cudaStream_t st) {
-    // (DG_HOST_MAX_PITCH in the environment lowers the limit: the tests use it to reach the per-row path at small sizes)
+    // (dg_host_set_max_pitch lowers the limit: the tests use it to reach the per-row path at small sizes)
     size_t limit = c.max_pitch;
-    if (const char* v = std::getenv("DG_HOST_MAX_PITCH")) {
-        const unsigned long long x = std::strtoull(v, nullptr, 10);
-        if (x < limit) limit = (size_t)x;
-    }
+    const size_t cap = g_pitch_cap.load(std::memory_order_relaxed);
+    if (cap != 0 && cap < limit) limit = cap;
     if (dpitch <= limit && spitch <= limit) return cudaMemcpy2DAsync(dst, dpitch, src, spitch, width, rows, kind, st);
     for (size_t r = 0; r < rows; ++r)
         DG_TRY(cudaMemcpyAsync(static_cast<char*>(dst) + r * dpitch, static_cast<const char*>(src) + r * spitch, width, kind, st));
@@ -179,4 +178,10 @@ extern "C" dg_status dg_host_release(void) {
     }
     cudaSetDevice(prev);
     return cuda_status(first);
+}
+
+extern "C" dg_status dg_host_set_max_pitch(long long bytes) {
+    if (bytes < 0) return DG_EINVAL;
+    g_pitch_cap.store((size_t)bytes, std::memory_order_relaxed);
+    return DG_OK;
 }

@@ -18,6 +18,8 @@
 // tiles in flight on all SMs stay L2-resident: with 2048-cell tiles they did not (5.6 KB of DRAM reads per cell for
 // 0.94 KB needed, ncu round 2), because a 32-byte sector fetched for one cell was evicted before its three neighbours
 // were processed.
+#include <atomic>
+
 #include "dg_internal.h"
 #include "dg_ppc.cuh"
 
@@ -44,6 +46,10 @@ struct Sched {  // block-wide scheduling state
     // One word, so that publishing a tile, claiming a chunk (compare-and-swap) and noticing that the buffer has moved on
     // to a later tile are each a single atomic access.
     unsigned state[kBufs];
+    // per buffer: how many claimed chunks of the tile in the buffer have READ their order[] entries.  A buffer is sorted
+    // into again only when every chunk of its previous tile has been counted here (sort_and_publish), so a claimer can
+    // never find a later tile's order under its feet, however long it is held up between its claim and its read.
+    unsigned done[kBufs];
 };
 static_assert(kTile / 16 < 256, "the chunk counter lives in the low byte of Sched::state");
 constexpr size_t kTilesBytes = Core::kWarpBytes * kWarps;
@@ -174,8 +180,21 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
         return left < kTile ? (int)left : kTile;
     };
     // sorts tile k into its buffer and publishes it (called by ONE warp, whose own tile is free at that moment)
+    auto chunks_of = [&](int k) { return (tile_count(k) + CW - 1) / CW; };
     auto sort_and_publish = [&](int k) {
         const int b = k % kBufs;
+        if (k >= kBufs) {
+            // The buffer still belongs to tile k - kBufs until all its chunks have read their cells from it.  (They were
+            // claimed at least a whole tile ago, so this wait is over before it starts; it is here so that the recycling
+            // is correct by construction and not by timing.  No deadlock: a warp counts its read before it claims again,
+            // and only a warp that has claimed chunk 0 of tile k - 1 gets here.)
+            if (lane == 0) {
+                const unsigned need = (unsigned)chunks_of(k - kBufs);
+                while (*reinterpret_cast<volatile unsigned*>(&sch.done[b]) < need) __nanosleep(32);
+                *reinterpret_cast<volatile unsigned*>(&sch.done[b]) = 0;  // nobody counts again before the publish below
+            }
+            __syncwarp();
+        }
         sort_tile_warp(G.rho_g, G.rho_d, G.t_s, G.dt, nc, N, tile_base(k), tile_count(k),
                        reinterpret_cast<unsigned*>(my_tile), sch.order[b], lane);
         __syncwarp();
@@ -184,7 +203,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
         __syncwarp();
     };
 
-    if (threadIdx.x < kBufs) sch.state[threadIdx.x] = 0;
+    if (threadIdx.x < kBufs) {
+        sch.state[threadIdx.x] = 0;
+        sch.done[threadIdx.x] = 0;
+    }
     __syncthreads();  // the only block-wide barrier
     if (warp == 0) sort_and_publish(0);
 
@@ -217,9 +239,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
             if (j < nchunks) {
                 const int pos = j * CW + c;
                 valid = pos < count;
-                // (the buffer cannot be recycled between the claim and this read: that takes two more tiles' worth of
-                // claims by the other warps and a sort, which starts with a round trip to HBM)
+                // Invariant: between a successful claim of a chunk of tile kc and the count below, buffer b holds tile
+                // kc's order — sort_and_publish(kc + kBufs) waits for done[b] to reach the tile's chunk count first.
+                __threadfence_block();  // the order[] entries were written before the state word this claim observed
                 cell = tile_base(kc) + (valid ? (int)*reinterpret_cast<volatile unsigned short*>(&sch.order[b][pos]) : 0);
+                __threadfence_block();  // ... and are read before this chunk is counted as done with the buffer
+                __syncwarp();
+                if (lane == 0) atomicAdd(&sch.done[b], 1u);
                 // the first claimer of a tile sorts the next one before it starts on its chunk
                 if (j == 0 && kc + 1 < ktiles) sort_and_publish(kc + 1);
                 return true;
@@ -247,8 +273,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                 {
                     // my own positions hold the dust species k = 2a + r: rows r, r + 2, ... of t_s and rho_d (running
                     // pointers; an inert slot re-reads the last live row)
-                    const double* pt = G.t_s + (long long)r * nc + cell;
-                    const double* pd = G.rho_d + (long long)r * nc + cell;
+                    const int r0 = r < N ? r : N - 1;  // (N = 1: role 1 owns no live species; row 1 does not exist)
+                    const double* pt = G.t_s + (long long)r0 * nc + cell;
+                    const double* pd = G.rho_d + (long long)r0 * nc + cell;
                     const long long step = 2 * nc;
                     static_for<0, g>([&](auto a) {
                         cp_async8(&Core::at(V, 2 * a, 2), pt);
@@ -426,12 +453,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
 }
 
 cudaError_t launch_update(const UpdateArgs& a, int N, cudaStream_t st) {
-    static long long cap[64] = {0};  // blocks per device (one per SM: the shared-memory tile fills it); 0 = not queried
+    // blocks per device (one per SM: the shared-memory tile fills it); 0 = not queried.  Atomic: the entry points may be
+    // called from several host threads at once (two may both run the query: harmless; a torn value is not).
+    static std::atomic<long long> cap[64];
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (cap[dev] == 0) {
+    long long blocks = cap[dev].load(std::memory_order_acquire);
+    if (blocks == 0) {
         int sms = 0, per_sm = 0;
         e = cudaFuncSetAttribute(k_update_ppc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
         if (e != cudaSuccess) return e;
@@ -439,10 +469,11 @@ cudaError_t launch_update(const UpdateArgs& a, int N, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update_ppc, kThreads, kSmemBytes);
         if (e != cudaSuccess) return e;
-        cap[dev] = (long long)sms * (per_sm > 0 ? per_sm : 1);
+        blocks = (long long)sms * (per_sm > 0 ? per_sm : 1);
+        cap[dev].store(blocks, std::memory_order_release);
     }
     const long long ntiles = (a.ncells + kTile - 1) / kTile;
-    k_update_ppc<<<(unsigned)(ntiles < cap[dev] ? ntiles : cap[dev]), kThreads, kSmemBytes, st>>>(a, N);
+    k_update_ppc<<<(unsigned)(ntiles < blocks ? ntiles : blocks), kThreads, kSmemBytes, st>>>(a, N);
     return cudaGetLastError();
 }
 

@@ -21,6 +21,7 @@
 // p_in and p_out, so the kinetic energies before and after the update (Eq. 4, R20) cost one more row (E) and a few
 // FMAs per species instead of two further passes over the momenta in HBM.
 // Unaligned pointers (8 but not 16 bytes), odd row strides and the ragged last tile take per-thread 8-byte copies.
+#include <atomic>
 #include <cstdint>
 
 #include "dg_internal.h"
@@ -50,10 +51,7 @@ constexpr int kWarps = kThreads / 32;
 // Tile size and resident blocks per SM, measured on B200 (2^22 stiff cells): 128-thread blocks with ONE
 // tile each beat larger blocks, larger tiles at fewer blocks per SM and blocks that walk several tiles with the next
 // tile's copies under way: what hides a block's load / sort / store phases is the other blocks on the SM.
-#if defined(DG_TPS_TILE) && defined(DG_TPS_MINBLOCKS)  // tuning experiments only
-constexpr int kTile = DG_TPS_TILE;
-constexpr int kMinBlocks = DG_TPS_MINBLOCKS;
-#elif defined(DG_TPS_F32)  // half the bytes and about half the registers per cell
+#if defined(DG_TPS_F32)  // half the bytes and about half the registers per cell
 constexpr int kTile = N <= 1 ? 128 : 256;
 constexpr int kMinBlocks = N <= 1 ? 16 : N <= 2 ? 14 : N <= 6 ? 6 : N <= 8 ? 4 : 3;
 #else
@@ -152,7 +150,10 @@ __device__ __forceinline__ int sort_key(Real norm) {
         return min(max(e + 32, 1), kKeys - 1);
     } else {
         const Real theta = Num<Real>::theta(kRows - 1);  // 3.54 (double), 6.32 (float): exponent 1, 2
-        if (norm <= theta) return max(20 + e - (sizeof(Real) == 8 ? 1 : 2), 1);  // s = 0
+        // s = 0.  A valid norm here has e <= theta's exponent, so the key is at most 20; the upper clamp is for a NEGATIVE
+        // norm (a cell that breaks the preconditions: t_s < 0, rho < 0), whose exponent can be anything: its key must stay
+        // inside seg[][] / base[] so that the damage stays in that cell (include/dg.h, "Pre-conditions").
+        if (norm <= theta) return min(max(20 + e - (sizeof(Real) == 8 ? 1 : 2), 1), 20);
         if (!(norm > theta)) return kKeys - 1;                                    // NaN
         return 20 + min(scaling_exponent(norm, theta), kKeys - 1 - 20);
     }
@@ -431,16 +432,18 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update_tps(Args g, Ene
 
 template <bool kEnergy>
 cudaError_t launch(const Args& a, const EnergyArgs& eg, cudaStream_t st) {
-    static bool configured[64] = {false};
+    // Per device: has the kernel been given its dynamic shared-memory size.  Atomic: the entry points may be called from
+    // several host threads at once (include/dg.h); setting the attribute twice is harmless, a torn flag is not.
+    static std::atomic<bool> configured[64];
     constexpr size_t smem = kSmemBytesT<kEnergy>;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (!configured[dev]) {
+    if (!configured[dev].load(std::memory_order_acquire)) {
         e = cudaFuncSetAttribute(k_update_tps<kEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured[dev] = true;
+        configured[dev].store(true, std::memory_order_release);
     }
     const long long ntiles = (a.ncells + kTile - 1) / kTile;
     if (ntiles > 0x7fffffffLL) return cudaErrorInvalidValue;

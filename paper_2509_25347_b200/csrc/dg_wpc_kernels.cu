@@ -7,6 +7,8 @@
 // matrix work of the current group starts; results are staged in shared memory (over the group's own momenta rows)
 // and written back as whole sectors.
 // There is no block-level synchronisation: warps are independent, __syncwarp is the only barrier.
+#include <atomic>
+
 #include "dg_internal.h"
 #include "dg_wpc.cuh"
 
@@ -311,13 +313,17 @@ __global__ void __launch_bounds__(kThreads) k_expm_wpc(ExpmArgs g) {
 }
 
 // Persistent grid: as many blocks as fit on the device at once (or fewer, if there is not enough work).  The
-// occupancy query and the shared-memory opt-in are done once per device and cached (`cap` = blocks per device).
-cudaError_t persistent_grid(const void* kernel, size_t smem, long long (&cap)[64], long long units, unsigned* grid) {
+// occupancy query and the shared-memory opt-in are done once per device and cached (`cap` = blocks per device; atomic,
+// because the entry points may be called from several host threads at once: two threads may both do the query, which is
+// harmless, but neither may see a torn value).
+using CapTable = std::atomic<long long>[64];
+cudaError_t persistent_grid(const void* kernel, size_t smem, CapTable& cap, long long units, unsigned* grid) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (cap[dev] == 0) {
+    long long blocks = cap[dev].load(std::memory_order_acquire);
+    if (blocks == 0) {
         int sms = 0, per_sm = 0;
         if (smem > 0) {
             e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -327,15 +333,16 @@ cudaError_t persistent_grid(const void* kernel, size_t smem, long long (&cap)[64
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kThreads, smem);
         if (e != cudaSuccess) return e;
-        cap[dev] = (long long)sms * (per_sm > 0 ? per_sm : 1);
+        blocks = (long long)sms * (per_sm > 0 ? per_sm : 1);
+        cap[dev].store(blocks, std::memory_order_release);
     }
     const long long want = (units + kWarps - 1) / kWarps;
-    *grid = (unsigned)(want < cap[dev] ? want : cap[dev]);
+    *grid = (unsigned)(want < blocks ? want : blocks);
     return cudaSuccess;
 }
 
 cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
-    static long long cap[64] = {0};  // per device; 0 = not yet queried
+    static CapTable cap;  // per device; 0 = not yet queried
     unsigned grid = 0;
     const long long ngroups = (a.ncells + kGroup - 1) / kGroup;
     cudaError_t e = persistent_grid((const void*)k_update_wpc, kSmemBytes, cap, ngroups, &grid);
@@ -344,7 +351,7 @@ cudaError_t launch_update(const UpdateArgs& a, cudaStream_t st) {
     return cudaGetLastError();
 }
 cudaError_t launch_expm(const ExpmArgs& a, cudaStream_t st) {
-    static long long cap[64] = {0};
+    static CapTable cap;
     unsigned grid = 0;
     cudaError_t e = persistent_grid((const void*)k_expm_wpc, 0, cap, a.ncells, &grid);
     if (e != cudaSuccess) return e;

@@ -207,7 +207,26 @@ def test_full_size_sampled(dg, oracle, cuda, config):
     # a strided sample plus the 256 stiffest cells of the whole array (largest ||A||_1: the most squarings)
     norm1 = 2.0 * torch.maximum((wl.rho_d / wl.rho_g[None, :] * (wl.dt / wl.t_s)).sum(dim=0), (wl.dt / wl.t_s).amax(dim=0))
     stiffest = torch.topk(norm1, 256).indices.cpu()
-    idx = torch.unique(torch.cat([W.sample_cells(wl.ncells, 2048), stiffest]))
+    # 2^18 sampled cells at full size, always including the 256 largest-norm cells
+    idx = torch.unique(torch.cat([W.sample_cells(wl.ncells, 2 ** 18), stiffest]))
+    run_and_compare(dg, oracle, wl, idx=idx)
+    out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    drift = (out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)
+    assert torch.isfinite(out).all()
+    assert float(drift.max()) <= CONS_TOL
+
+
+@pytest.mark.parametrize("N", [4, 12, 13, 16])
+def test_sweep_size_sampled(dg, oracle, cuda, N):
+    """BASELINE.json configs[4] at its own size (2^22 stiff cells), for both default kernel families at their smallest and
+    largest species counts (sorted tiles: N = 4, 12; pair per cell: N = 13, 16): the grids, the tile walk and the bulk-copy
+    alignment of the launch bench.py times, which the few-thousand-cell tests never reach.  2^16 sampled cells plus the
+    256 stiffest against the oracle, conservation on every cell."""
+    wl = W.make_workload(5, N=N, device=cuda)
+    assert wl.ncells == 2 ** 22
+    norm1 = 2.0 * torch.maximum((wl.rho_d / wl.rho_g[None, :] * (wl.dt / wl.t_s)).sum(dim=0), (wl.dt / wl.t_s).amax(dim=0))
+    stiffest = torch.topk(norm1, 256).indices.cpu()
+    idx = torch.unique(torch.cat([W.sample_cells(wl.ncells, 2 ** 16), stiffest]))
     run_and_compare(dg, oracle, wl, idx=idx)
     out = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
     drift = (out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)
@@ -409,9 +428,12 @@ def test_pair_per_cell_scheduler_with_wildly_uneven_tiles(dg, oracle, cuda, N):
     """The pair-per-cell kernel hands out chunks of sorted 128-cell tiles to its warps through a small lock-free queue
     (three order buffers per block).  Whole tiles of trivially cheap cells (dt/t_s ~ 1e-9: s = 0, m = 2) next to tiles of
     very stiff ones (dt/t_s ~ 1e8: s ~ 30) make some warps fall several tiles behind the others — the situation in which a
-    lagging warp meets a recycled buffer.  Few enough cells that one block walks many tiles.  Must terminate, match the
-    oracle where it can referee (||A||_1 <= 1e6) and conserve momentum everywhere."""
-    ncells = 128 * 61 + 37
+    lagging warp meets a recycled buffer (a buffer is re-sorted only once every chunk of its previous tile has read its
+    cells from it: Sched::done in dg_ppc_kernels.cu).  The kernel launches one block per SM, so the cell count is taken
+    from the device: every block walks at least 8 tiles and recycles each of its three buffers at least twice.  Must
+    terminate, match the oracle on EVERY cell it can referee (||A||_1 <= 1e6) and conserve momentum everywhere."""
+    sms = torch.cuda.get_device_properties(cuda).multi_processor_count
+    ncells = 128 * sms * 8 + 37
     wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
     tile = torch.arange(ncells, device=cuda) // 128
     cheap = (tile % 3 != 1)
@@ -529,6 +551,44 @@ def test_non_finite_input_stays_in_its_cell(dg, oracle, cuda, N, variant):
     for c in (7, 40, 150, 299):
         assert not bool(torch.isfinite(out[:, :, c]).all()), c
     assert not bool(torch.isfinite(out[1, :, 41]).all()) and bool(torch.isfinite(out[0, :, 41]).all())
+
+
+@pytest.mark.parametrize("N", [1, 4, 8, 9, 12, 13, 16])
+def test_negative_input_stays_in_its_cell(dg, oracle, cuda, N):
+    """include/dg.h, 'Pre-conditions': a cell that breaks them (here: negative stopping times and densities, e.g. a
+    -1e30 fill value, or t_s = -0.0 whose reciprocal is -Inf) may come back meaningless, but only that cell.  A negative
+    norm bound has an arbitrary binary exponent; the sorted-tile kernels turn the exponent into a shared-memory index
+    (N = 9..12 through the squarings key), so this is an out-of-bounds check as much as a numerical one.  Default kernels,
+    double and single precision."""
+    wl = W.make_workload(5, ncells=700, N=N, device=cuda)
+    clean64 = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    f = lambda t: t.to(torch.float32)
+    clean32 = dg.dg_drag_update_f32(f(wl.rho_g), f(wl.rho_d), f(wl.t_s), wl.dt, f(wl.p_in))[0]
+    bad = [3, 64, 65, 300, 511, 699]
+    wl.t_s[0, 3] = -1e-300            # a = dt / t_s = -huge: exponent ~ +996
+    wl.t_s[N - 1, 64] = -0.0          # a = -Inf
+    wl.rho_d[0, 65] = -1e30           # eps < 0: the norm bound goes negative
+    wl.rho_g[300] = -1e-30            # eps = -huge
+    wl.t_s[:, 511] = -1e-30
+    wl.rho_d[:, 699] = -1e300
+    out64 = dg.dg_drag_update(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    out32 = dg.dg_drag_update_f32(f(wl.rho_g), f(wl.rho_d), f(wl.t_s), wl.dt, f(wl.p_in))[0]
+    torch.cuda.synchronize()
+    good = torch.ones(wl.ncells, dtype=torch.bool)
+    good[bad] = False
+    idx = torch.nonzero(good).flatten()
+    rho_g, rho_d, t_s, p_in = wl.cells(idx)
+    ref = oracle.drag_update(rho_g, rho_d, t_s, wl.dt, p_in)
+    got = out64[:, :, idx.to(cuda)].cpu().numpy()
+    assert np.isfinite(got).all()
+    assert float(oracle.parity_error(got, ref, p_in).max()) <= PARITY_TOL
+    # single precision: the healthy cells stay where the clean run put them (to rounding: the warp's Taylor degree may
+    # differ when a poisoned cell shares the chunk)
+    g = idx.to(cuda)
+    scale = wl.p_in.abs().amax(dim=(0, 1))[g].to(torch.float32)
+    assert bool(torch.isfinite(out32[:, :, g]).all())
+    assert float(((out32[:, :, g] - clean32[:, :, g]).abs().amax(dim=(0, 1)) / scale).max()) <= 1e-4
+    assert float(((out64[:, :, g] - clean64[:, :, g]).abs().amax(dim=(0, 1)) / scale.double()).max()) <= 2 * PARITY_TOL
 
 
 @pytest.mark.parametrize("N,ncells", [(1, 33), (4, 127), (8, 1001), (13, 130), (16, 1027), (16, 3), (2, 512), (8, 1026),
@@ -670,13 +730,12 @@ def test_host_entry_point_matches_device_entry_point(dg, cuda, N, ncells, chunk)
     dg.dg_drag_update_host(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, p, p_out=p, chunk_cells=chunk)
     assert torch.equal(p, out_h)
     # rows wider than a 2-D copy's pitch limit (ncells >= 2^28 in real life) go one 1-D copy per row: forced here by
-    # lowering the limit through the environment
-    import os
-    os.environ["DG_HOST_MAX_PITCH"] = "1024"
+    # lowering the limit through the library's test hook
+    dg.dg_host_set_max_pitch(1024)
     try:
         out_rows = dg.dg_drag_update_host(h[0], h[1], h[2], wl.dt, h[3], chunk_cells=chunk)
     finally:
-        del os.environ["DG_HOST_MAX_PITCH"]
+        dg.dg_host_set_max_pitch(0)
     assert torch.equal(out_rows, out_h)
     dg.dg_host_release()
 
