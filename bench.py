@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — drag-update throughput (cells/s, fp64) of the fused CUDA path, with its roofline and the CPU oracle.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--no-sweep] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--no-sweep] [--legs] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (a1..a5) over one batch of synthetic input = ONE
 dg_drag_update launch over all cells of the workload.  Inputs are resident in HBM when the timed region starts;
@@ -10,8 +10,14 @@ L2, so no L2 flush is needed between iterations.  Timing: CUDA events on the lau
 synchronize on both sides, max over ranks.  --gpus N > 1 runs N independent replicas (the path does not
 shard, there is no collective on the data path); value = cells all ranks processed / max time.
 
-Prints ONE JSON line (rank 0).  Keys beyond the base contract: roofline, cpu_baseline, e2e, clocks, gpu_launches,
-peaks (the microbenchmarked denominators), sweep (the other BASELINE.json configs, device-timed the same way).
+Prints ONE short, strict-JSON line (rank 0; the last line of stdout, under 4 KB).  Keys beyond the base contract:
+roofline, cpu_baseline, e2e, clocks, gpu_launches, peaks (the microbenchmarked denominators), ms_per_launch
+(min / median / max over the timed launches), repeat_ms_per_step (two more timed regions of the same length: the
+run-to-run spread) and a compact sweep (the other BASELINE.json configs, device-timed the same way: workload,
+ms_per_step, bound, frac, timed_launches).  Everything else — the full per-workload records and, with --legs, the RK1 /
+energy / single-precision / paper-as-printed measurements on the same buffers — goes to --detail-file
+(default gpurun_out/bench_detail.json), never to stdout.
+The default workload is BASELINE.json configs[3] (N = 16, 256^3 cells): the largest single-GPU configuration.
 --impl reference times the CPU oracle (oracle/) on the host cores on the same workload recipe.
 """
 import argparse
@@ -328,15 +334,17 @@ def run_reference(args):
         dgo.drag_update(cells[0], cells[1], cells[2], wl.dt, cells[3])
     sec = time.perf_counter() - t0
     value = len(idx) * args.steps / sec
-    sample = f"{len(idx)} cells per step strided over the first {wl.ncells} cells of the recipe"
+    full_cells = W.CONFIG_CELLS[args.config]
+    sample = (f"{len(idx)} cells per step, strided over a {wl.ncells}-cell draw of the same recipe "
+              f"(the workload itself has {full_cells} cells)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
-        "config": {"workload": wl.name.split("_")[0] + f"_N{wl.N}", "recipe": f"BASELINE.json configs[{args.config - 1}]",
-                   "sample": sample},
+        "config": {"workload": f"config{args.config}_N{wl.N}_{full_cells}cells",
+                   "recipe": f"BASELINE.json configs[{args.config - 1}]", "N": wl.N, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}, allow_nan=False))
 
 
 def bench_rk1(dg, wl, p_out, hbm_gbs, steps=5, warmup=3):
@@ -450,7 +458,7 @@ def bench_paper_variant(dg, wl, p_out, steps=2, warmup=1):
     return res
 
 
-def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None, min_region_ms=0.0):
+def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None, min_region_ms=0.0, legs=False, repeats=0):
     """One workload, device-timed.  min_region_ms > 0 (the sweep entries): the number of timed launches is raised (up to
     400) until the timed region lasts about that long, and no event is recorded between launches — a 0.1 ms kernel timed
     over five launches with an event after each reads 5-8 % slow (launch latency after the synchronize, event gaps)."""
@@ -467,21 +475,50 @@ def bench_one(dg, wl, steps, warmup, peaks, hbm_gbs, hbm_src, sampler=None, min_
     flops = useful_flops(wl.N, s, m)
     ms_launch = sum(per) / len(per)
     roof = roofline_for(wl, ms_launch, dense_flops, flops, peaks, hbm_gbs, hbm_src)
+    sp = sorted(per)
     res = {"workload": wl.name, "N": wl.N, "ncells": wl.ncells, "ms_per_step": total_ms / steps,
-           "ms_per_launch_min": min(per), "timed_launches": steps, "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
+           # per-launch figures exist only where an event was recorded after every launch (not in the sweep entries)
+           "ms_per_launch": {"min": sp[0], "median": sp[len(sp) // 2], "max": sp[-1]} if fine else None,
+           "timed_launches": steps, "cells_per_s": wl.ncells * steps / (total_ms * 1e-3),
            "useful_flops_per_cell": flops / wl.ncells, "dense_flops_per_cell": dense_flops / wl.ncells,
            "dense_products_per_cell": products, "algorithmic_bytes_per_cell": algorithmic_bytes_per_cell(wl.N),
            "mean_s": float(s.double().mean().item()), "mean_m": float(m.double().mean().item()),
            "max_s": int(s.max().item()), "roofline": roof, "variant": dg.dg_variant_name(wl.N)}
-    res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs, steps=5 if fine else max(5, steps))   # same timed-region rule
-    res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
-    if wl.ncells <= (1 << 22):   # the two rank-4 entry points, on the 2^21..2^22-cell workloads (they need extra buffers)
-        res["energy"] = bench_energy(dg, wl, p_out, ms_launch, hbm_gbs)
-        res["f32"] = bench_f32(dg, wl, ms_launch, 2.0 * peaks["fp64_nominal_tflops"])   # 128 fp32 vs 64 fp64 FMA lanes per SM
-    res["paper_as_printed"] = bench_paper_variant(dg, wl, p_out)
-    res["paper_as_printed"]["speedup_of_product_path"] = res["paper_as_printed"]["ms_per_launch"] / ms_launch
+    # the run-to-run spread: further timed regions of the same length, after the one the headline is taken from
+    res["repeat_ms_per_step"] = [time_device_steps(dg, wl, p_out, steps, 1, None, per_launch_events=fine)[0] / steps
+                                 for _ in range(repeats)]
+    if legs:   # --legs: the SURVEY.md §8(f) entry points on the same buffers (detail file only)
+        res["rk1"] = bench_rk1(dg, wl, p_out, hbm_gbs, steps=5 if fine else max(5, steps))   # same timed-region rule
+        res["rk1"]["exp_over_rk1_time"] = ms_launch / res["rk1"]["ms_per_launch"]
+        if wl.ncells <= (1 << 22):   # the two rank-4 entry points, on the 2^21..2^22-cell workloads (they need extra buffers)
+            res["energy"] = bench_energy(dg, wl, p_out, ms_launch, hbm_gbs)
+            res["f32"] = bench_f32(dg, wl, ms_launch, 2.0 * peaks["fp64_nominal_tflops"])   # 128 fp32 vs 64 fp64 FMA lanes per SM
+        res["paper_as_printed"] = bench_paper_variant(dg, wl, p_out)
+        res["paper_as_printed"]["speedup_of_product_path"] = res["paper_as_printed"]["ms_per_launch"] / ms_launch
     del p_out
     return res, total_ms
+
+
+def _strict(x):
+    """A copy of x that json.dumps(..., allow_nan=False) accepts: non-finite floats become None."""
+    if isinstance(x, float):
+        return x if math.isfinite(x) else None
+    if isinstance(x, dict):
+        return {k: _strict(v) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_strict(v) for v in x]
+    return x
+
+
+def _rounded(x, digits=6):
+    """Floats to `digits` significant digits (the printed line only: the detail file keeps full precision)."""
+    if isinstance(x, float):
+        return float(f"{x:.{digits}g}") if math.isfinite(x) else x
+    if isinstance(x, dict):
+        return {k: _rounded(v, digits) for k, v in x.items()}
+    if isinstance(x, (list, tuple)):
+        return [_rounded(v, digits) for v in x]
+    return x
 
 
 def main():
@@ -490,12 +527,15 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[config-1]; 5 = sweep point (give --N)")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs[config-1] (default 4: N = 16, 256^3, the "
+                    "largest single-GPU configuration); 5 = sweep point (give --N)")
     ap.add_argument("--N", type=int, default=None)
     ap.add_argument("--variant", type=int, default=0, help="force a mapping: 1 thread/cell, 2 warp/cell DMMA, 4 pair/cell")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--legs", action="store_true", help="also time RK1 / energy / f32 / paper-as-printed (detail file only)")
+    ap.add_argument("--detail-file", default=os.path.join(ROOT, "gpurun_out", "bench_detail.json"))
     args = ap.parse_args()
     if args.config == 5 and args.N is None:
         args.N = 16
@@ -526,7 +566,8 @@ def main():
     # replicas: every rank runs the same recipe with its own seed
     wl = W.make_workload(args.config, N=args.N, device=device, seed=rank)
     clk = ClockSampler(local_rank)
-    res, total_ms = bench_one(dg, wl, args.steps, args.warmup, peaks, hbm_gbs, hbm_src, sampler=clk)
+    res, total_ms = bench_one(dg, wl, args.steps, args.warmup, peaks, hbm_gbs, hbm_src, sampler=clk, legs=args.legs,
+                              repeats=2)
     clocks = clk.summary()
     ms_max, cells_all = aggregate_over_ranks(total_ms, wl.ncells * args.steps)
     value = cells_all / (ms_max * 1e-3)
@@ -563,27 +604,50 @@ def main():
         points = [(c, None) for c in (2, 3, 4) if c != args.config] + [(5, N) for N in W.SWEEP_N]
         for cfg, N in points:
             w2 = W.make_workload(cfg, N=N, device=device)
-            r2, _ = bench_one(dg, w2, max(3, min(args.steps, 5)), 3, peaks, hbm_gbs, hbm_src, min_region_ms=20.0)
+            r2, _ = bench_one(dg, w2, max(3, min(args.steps, 5)), 3, peaks, hbm_gbs, hbm_src, min_region_ms=20.0,
+                              legs=args.legs)
             sweep.append(r2)
             del w2
             torch.cuda.empty_cache()
 
     if rank == 0:
+        roof = res["roofline"]
+        short_roof = {k: roof.get(k) for k in ("bound", "achieved", "peak", "unit", "frac", "traffic", "algorithmic_bytes")}
+        short_roof["peak_source"] = ("nominal fp64 FMA peak = SMs x 64 lanes x 2 x clocks.max.sm (DESIGN.md §6)"
+                                     if roof["bound"] == "alu" else hbm_src)
+        if roof["bound"] == "alu":
+            short_roof["flops_per_cell"] = res["useful_flops_per_cell"]
+            short_roof["frac_of_measured_dfma"] = roof["frac_of_measured_dfma"]
+            short_roof["dense_equivalent_frac"] = roof["dense_equivalent"]["frac"]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": res["workload"], "recipe": f"BASELINE.json configs[{args.config - 1}]",
                        "N": res["N"], "ncells_per_gpu": res["ncells"], "parallelism": "replicas" if world > 1 else "1 GPU",
-                       "l2": "inputs larger than L2 (no flush)", "variant": res["variant"],
-                       "paper_context": "A100/Dyablo N=8: 9.7e-9 s/cell = 1.03e8 cells/s (PAPER.md:341); other machine"},
-            "roofline": res["roofline"], "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+                       "l2": "inputs larger than L2 (no flush)", "variant": res["variant"]},
+            "roofline": short_roof, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
             "gpu_launches": args.steps * dg.dg_launches_per_update(res["N"], res["ncells"]),
+            "ms_per_launch": res["ms_per_launch"], "repeat_ms_per_step": res["repeat_ms_per_step"],
             "peaks": dict(peaks, hbm_gbs=hbm_gbs, hbm_source=hbm_src, gpu=props.name, sms=props.multi_processor_count),
-            "detail": {k: v for k, v in res.items() if k not in ("roofline",)},
-            "sweep": sweep,
+            "sweep": [{"workload": r["workload"], "ms_per_step": r["ms_per_step"], "bound": r["roofline"]["bound"],
+                       "frac": r["roofline"]["frac"], "timed_launches": r["timed_launches"]} for r in sweep],
         }
-        print(json.dumps(line))
+        line = _strict(_rounded(line))
+        detail = _strict({"line": line, "headline": res, "sweep": sweep,
+                          "paper_context": "A100/Dyablo N=8: 9.7e-9 s/cell = 1.03e8 cells/s (PAPER.md:341); other machine"})
+        try:
+            os.makedirs(os.path.dirname(args.detail_file), exist_ok=True)
+            with open(args.detail_file, "w") as f:
+                json.dump(detail, f, indent=1, allow_nan=False)
+        except OSError as e:   # a read-only checkout must not cost the headline
+            print(f"bench.py: could not write {args.detail_file}: {e}", file=sys.stderr)
+        text = json.dumps(line, allow_nan=False, separators=(",", ":"))
+        if len(text) > 4000:   # the driver keeps only the tail of stdout: the sweep is in the detail file anyway
+            line["sweep"] = []
+            text = json.dumps(line, allow_nan=False, separators=(",", ":"))
+        sys.stdout.flush()
+        print(text, flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
