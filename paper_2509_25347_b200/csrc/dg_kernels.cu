@@ -2,6 +2,7 @@
 //
 // Thread-per-cell kernels: every field is structure-of-arrays with the cell index fastest, so a warp's loads and
 // stores of one field row are 256 contiguous bytes.  The fused kernel k_update never writes a matrix to HBM.
+#include "dg_async.cuh"
 #include "dg_internal.h"
 #include "dg_tpc.cuh"
 
@@ -31,16 +32,6 @@ constexpr int kMinBlocks = N <= 2 ? 8 : N <= 4 ? 4 : N <= 7 ? 3 : 2;  // registe
 constexpr int kRowsIn = 1 + 2 * N;  // rho_g, rho_d[N], t_s[N]
 constexpr int kRowsP = 3 * n;       // p_in[3][n]
 constexpr size_t kSmemBytes = (size_t)(kRowsIn + kRowsP) * kThreads * sizeof(double);
-
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int Pending>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(Pending) : "memory");
-}
 
 __global__ void __launch_bounds__(kThreads, kMinBlocks) k_update(UpdateArgs g) {
     extern __shared__ double stage[];

@@ -20,6 +20,7 @@
 // were processed.
 #include <atomic>
 
+#include "dg_async.cuh"
 #include "dg_internal.h"
 #include "dg_ppc.cuh"
 
@@ -65,16 +66,9 @@ __device__ __forceinline__ double ldg_now(const double* p) {
     asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
-// Asynchronous 8-byte copy global -> shared (LDGSTS).  The gathers of a chunk are issued back to back through these
-// and waited for ONCE: with plain loads ptxas places each dependent reciprocal right behind its load, and the warp
+// (cp_async8 of dg_async.cuh: asynchronous 8-byte copy global -> shared, LDGSTS.)  The gathers of a chunk are issued
+// back to back through it and waited for ONCE: with plain loads ptxas places each dependent reciprocal right behind its load, and the warp
 // (in-order issue) then pays one round trip to L2 per field row — 17 of them per chunk (ncu, round 2).
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() {
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
-}
 
 // One warp sorts the tile starting at cell `base` (count cells) into order[]: key = the squarings the norm bound
 // max_i a_i + sum_i eps_i a_i (R5) needs with the m = 30 row (its binary exponent below the last threshold), stiffest first, non-finite first of all, ties in cell order; entries

@@ -24,6 +24,7 @@
 #include <atomic>
 #include <cstdint>
 
+#include "dg_async.cuh"
 #include "dg_internal.h"
 #include "dg_tpc.cuh"
 
@@ -86,18 +87,6 @@ struct EnergyArgs {  // dg_drag_update_energy: E_in, E_out [ncells], heating fra
 template <bool kEnergy>
 constexpr size_t kSmemBytesT = sizeof(SmemT<kEnergy>);
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src_gmem) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async8(float* dst_smem, const float* src_gmem) {  // (one element: 4 bytes)
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int Pending>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(Pending) : "memory");
-}
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }

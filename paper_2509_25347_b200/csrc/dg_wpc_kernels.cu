@@ -9,6 +9,7 @@
 // There is no block-level synchronisation: warps are independent, __syncwarp is the only barrier.
 #include <atomic>
 
+#include "dg_async.cuh"
 #include "dg_internal.h"
 #include "dg_wpc.cuh"
 
@@ -40,20 +41,6 @@ struct alignas(16) WarpSmem {
 };
 static_assert(sizeof(WarpSmem) % 16 == 0, "cp.async 16-byte destinations need 16-byte aligned per-warp tiles");
 constexpr size_t kSmemBytes = sizeof(WarpSmem) * kWarps;
-
-__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async8(void* dst_smem, const void* src_gmem) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(src_gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int Pending>
-__device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(Pending) : "memory");
-}
 
 __device__ __forceinline__ const double* row_ptr(const UpdateArgs& g, int r) {
     const long long nc = g.ncells;
