@@ -129,7 +129,7 @@ dg_status dg_drag_rk1(const double* rho_g, const double* rho_d, const double* t_
  * fraction w (0 = no frictional heating, 1 = all of it) is deposited into the gas.  With w = 1,
  * E_g + sum_i |M_d,i|^2/(2 rho_d,i) is conserved.  A species with rho_d,i = 0 carries no energy.
  * in : rho_g, rho_d, t_s, p_in, E_in [ncells] (device), dt, w.   out: p_out (may alias p_in), E_out [ncells] (may alias
- * E_in).  One launch on `stream` for N <= 12 (the sums are formed inside the update kernel), three for N >= 13.
+ * E_in).  One launch on `stream` for every N (the sums are formed inside the update kernel).
  * DG_EINVAL if w is outside [0, 1]; otherwise the errors of dg_drag_update. */
 dg_status dg_drag_update_energy(const double* rho_g, const double* rho_d, const double* t_s, double dt,
                                 const double* p_in, const double* E_in, double w, int N, long long ncells,
@@ -238,8 +238,8 @@ dg_status dg_drag_update_host_static(const double* rho_g, const double* rho_d, c
 dg_status dg_peak_kernel(int kind, int iters, double* scratch, long long scratch_bytes, double* work, void* stream);
 
 /* Number of kernels ONE call of dg_drag_update (or _ex, _variant, _f32, _rk1) enqueues for these arguments: 1, or 0
- * if ncells == 0.  Not for the other entry points: dg_drag_update_steps enqueues nsteps times as many,
- * dg_drag_update_energy 1 for N <= 12 and 3 above, dg_drag_update_host one per chunk. */
+ * if ncells == 0 (dg_drag_update_energy likewise).  Not for the other entry points: dg_drag_update_steps enqueues
+ * nsteps times as many, dg_drag_update_host one per chunk. */
 int dg_launches_per_update(int N, long long ncells);
 /* Human-readable description of the kernel variant dg_drag_update uses for N (static storage). */
 const char* dg_variant_name(int N);

@@ -91,9 +91,9 @@ cudaError_t launch_update(int N, int variant, const UpdateArgs& a, cudaStream_t 
     return variant == DG_VARIANT_WPC ? kWpcTable[N]->update(a, st) : kTable[N]->update(a, st);
 }
 
-// dg_drag_update_energy in one launch, where the default kernel for N has a fused form (sorted tiles, N <= 12)
-bool has_fused_energy(int N) { return default_variant(N) == DG_VARIANT_TPS; }
+// dg_drag_update_energy: one launch of the default kernel for N, which forms the kinetic-energy sums on the way
 cudaError_t launch_update_energy(int N, const UpdateArgs& a, const double* E_in, double* E_out, double w, cudaStream_t st) {
+    if (default_variant(N) == DG_VARIANT_PPC) return kPpcTable[N]->update_energy(a, N, E_in, E_out, w, st);
     return kTpsTable[N]->update_energy(a, E_in, E_out, w, st);
 }
 

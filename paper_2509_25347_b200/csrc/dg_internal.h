@@ -74,6 +74,8 @@ struct PaperLaunchers {
 // Pair-per-cell kernel (dg_ppc_kernels.cu, one translation unit per EVEN number of dust slots NP; serves N = NP - 1, NP).
 struct PpcLaunchers {
     cudaError_t (*update)(const UpdateArgs&, int N, cudaStream_t);
+    // dg_drag_update_energy in ONE launch (s_out / m_out unused), as TpsLaunchers::update_energy
+    cudaError_t (*update_energy)(const UpdateArgs&, int N, const double* E_in, double* E_out, double w, cudaStream_t);
     int tile;  // cells per sorted tile: launches over sub-ranges that start on a multiple of it give the same bits
     const char* variant;
 };

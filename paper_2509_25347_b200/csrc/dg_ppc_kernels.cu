@@ -154,7 +154,16 @@ __device__ __noinline__ void sort_tile_warp(const double* rho_g, const double* r
     for (int j = 0; j < kPerLane; ++j) order[lane + j * 32] = (unsigned short)(mine[j] & 0xffffu);
 }
 
-__global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N) {
+// kEnergy: dg_drag_update_energy in the same launch — the two kinetic-energy sums of Eq. 4's drag part (dg_energy.cu) are
+// formed in the apply step, where a lane holds p_in and p_out of its own rows anyway; the plain instantiation carries
+// none of it.
+struct EnergyArgs {  // E_in, E_out [ncells], heating fraction w
+    const double* E_in;
+    double* E_out;
+    double w;
+};
+template <bool kEnergy>
+__global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N, EnergyArgs eg) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* tiles = reinterpret_cast<double*>(smem_raw);
     Sched& sch = *reinterpret_cast<Sched*>(smem_raw + kTilesBytes);
@@ -397,17 +406,33 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                 const long long comp_stride = (long long)n * nc;
                 // my own dust rows, species k = 2a + r; the row's p_in values are requested two rows ahead (they were read
                 // once for q, but a gather of 27 rows does not survive in what is left of L1 beside the 217 KB of tiles)
-                auto load_p = [&](int a, double (&pv)[3]) {
+                // (energy variant: rho_d of the row travels with its momenta, `prd` below)
+                const double* prd = G.rho_d + (long long)r * nc + cell;  // rho_d of my own row a: prd[2a nc]
+                auto load_p = [&](int a, double (&pv)[3], double& rv) {
                     const bool live = valid && 2 * a + r < N;
                     static_for<0, 3>([&](auto cp) { pv[cp] = live ? pin[(long long)(2 * a) * nc + cp * comp_stride] : 0.0; });
+                    if constexpr (kEnergy) rv = live ? prd[(long long)(2 * a) * nc] : 0.0;
                 };
-                double pa[3], pb[3];
-                load_p(0, pa);
-                load_p(g > 1 ? 1 : 0, pb);
-                auto row = [&](int a, const double (&pc)[3], const double (&y)[3]) {
+                double pa[3], pb[3], ra = 0.0, rb = 0.0;
+                load_p(0, pa, ra);
+                load_p(g > 1 ? 1 : 0, pb, rb);
+                // (energy variant) this lane's share of sum_i |M_d,i|^2 / (2 rho_d,i) before and after the step
+                double kd_in = 0.0, kd_out = 0.0;
+                auto row = [&](int a, const double (&pc)[3], double rd, const double (&y)[3]) {
                     const double w = V.x[((2 * a) * Core::ROW + Core::CWT) * CW];
                     if (valid && 2 * a + r < N) {
-                        static_for<0, 3>([&](auto cp) { pout[cp * comp_stride] = fma(w, y[cp], pc[cp]); });
+                        double po[3];
+                        static_for<0, 3>([&](auto cp) {
+                            po[cp] = fma(w, y[cp], pc[cp]);
+                            pout[cp * comp_stride] = po[cp];
+                        });
+                        if constexpr (kEnergy) {
+                            // 1 / (2 rho_d): true division, once per species and cell; a species with rho_d = 0 carries
+                            // no energy
+                            const double h = rd > 0.0 ? 0.5 / rd : 0.0;
+                            kd_in = fma(fma(pc[0], pc[0], fma(pc[1], pc[1], pc[2] * pc[2])), h, kd_in);
+                            kd_out = fma(fma(po[0], po[0], fma(po[1], po[1], po[2] * po[2])), h, kd_out);
+                        }
                     }
                     pout += 2 * nc;
                 };
@@ -419,25 +444,45 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
                         pc0[cp] = pa[cp];
                         pc1[cp] = pb[cp];
                     });
-                    load_p(a + 2 < g ? a + 2 : g - 1, pa);
-                    load_p(a + 3 < g ? a + 3 : g - 1, pb);
+                    const double rc0 = ra, rc1 = rb;
+                    load_p(a + 2 < g ? a + 2 : g - 1, pa, ra);
+                    load_p(a + 3 < g ? a + 3 : g - 1, pb, rb);
                     Core::apply_row(V, c_tab.ap[a], q, q0, y0);
                     Core::apply_row(V, c_tab.ap[a + 1], q, q0, y1);
-                    row(a, pc0, y0);
-                    row(a + 1, pc1, y1);
+                    row(a, pc0, rc0, y0);
+                    row(a + 1, pc1, rc1, y1);
                 }
                 if constexpr (g % 2 == 1) {
                     double y[3];
                     Core::apply_row(V, c_tab.ap[g - 1], q, q0, y);
-                    row(g - 1, pa, y);
+                    row(g - 1, pa, ra, y);
                 }
                 {  // the gas row (both lanes compute it, role 0 stores it)
+                    double rgv = 1.0;
+                    if constexpr (kEnergy) rgv = G.rho_g[cell];  // (requested before the row's arithmetic)
                     double y[3];
                     Core::apply_row(V, c_tab.ap[g], q, q0, y);
                     if (valid && r == 0) {
                         static_for<0, 3>([&](auto cp) {
                             G.p_out[cp * comp_stride + cell] = q0[cp] + y[cp];  // q0 is the gas momentum itself (w_z = 1)
                         });
+                    }
+                    if constexpr (kEnergy) {
+                        // E_g(t+dt) = E_g(t) + [KE_g(t+dt) - KE_g(t)] + w [K(t) - K(t+dt)],  K = KE_g + sum_i |M_d,i|^2 / (2 rho_d,i)
+                        // (dg_energy.cu).  The dust sums of the two lanes are added in role order; role 0 stores.
+                        const double oi = __shfl_xor_sync(kFullMask, kd_in, 16), oo = __shfl_xor_sync(kFullMask, kd_out, 16);
+                        if (valid && r == 0) {
+                            const double h = 0.5 / rgv;
+                            double g2_in = 0.0, g2_out = 0.0;
+                            static_for<0, 3>([&](auto cp) {
+                                const double po = q0[cp] + y[cp];
+                                g2_in = fma(q0[cp], q0[cp], g2_in);
+                                g2_out = fma(po, po, g2_out);
+                            });
+                            const double keg_in = g2_in * h, keg_out = g2_out * h;
+                            const double k_in = keg_in + (kd_in + oi), k_out = keg_out + (kd_out + oo);
+                            eg.E_out[cell] = eg.E_in[cell] + ((keg_out - keg_in) + eg.w * (k_in - k_out));
+                        }
                     }
                 }
             }
@@ -446,7 +491,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_update_ppc(UpdateArgs G, int N)
     }
 }
 
-cudaError_t launch_update(const UpdateArgs& a, int N, cudaStream_t st) {
+template <bool kEnergy>
+cudaError_t launch(const UpdateArgs& a, int N, const EnergyArgs& eg, cudaStream_t st) {
     // blocks per device (one per SM: the shared-memory tile fills it); 0 = not queried.  Atomic: the entry points may be
     // called from several host threads at once (two may both run the query: harmless; a torn value is not).
     static std::atomic<long long> cap[64];
@@ -457,25 +503,31 @@ cudaError_t launch_update(const UpdateArgs& a, int N, cudaStream_t st) {
     long long blocks = cap[dev].load(std::memory_order_acquire);
     if (blocks == 0) {
         int sms = 0, per_sm = 0;
-        e = cudaFuncSetAttribute(k_update_ppc, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        e = cudaFuncSetAttribute(k_update_ppc<kEnergy>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
         if (e != cudaSuccess) return e;
         e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update_ppc, kThreads, kSmemBytes);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update_ppc<kEnergy>, kThreads, kSmemBytes);
         if (e != cudaSuccess) return e;
         blocks = (long long)sms * (per_sm > 0 ? per_sm : 1);
         cap[dev].store(blocks, std::memory_order_release);
     }
     const long long ntiles = (a.ncells + kTile - 1) / kTile;
-    k_update_ppc<<<(unsigned)(ntiles < blocks ? ntiles : blocks), kThreads, kSmemBytes, st>>>(a, N);
+    k_update_ppc<kEnergy><<<(unsigned)(ntiles < blocks ? ntiles : blocks), kThreads, kSmemBytes, st>>>(a, N, eg);
     return cudaGetLastError();
+}
+cudaError_t launch_update(const UpdateArgs& a, int N, cudaStream_t st) {
+    return launch<false>(a, N, EnergyArgs{nullptr, nullptr, 0.0}, st);
+}
+cudaError_t launch_update_energy(const UpdateArgs& a, int N, const double* E_in, double* E_out, double w, cudaStream_t st) {
+    return launch<true>(a, N, EnergyArgs{E_in, E_out, w}, st);
 }
 
 }  // namespace
 
 #define DG_CAT_(a, b) a##b
 #define DG_CAT(a, b) DG_CAT_(a, b)
-extern const PpcLaunchers DG_CAT(ppc_launchers_NP, DG_NP) = {launch_update, kTile,
+extern const PpcLaunchers DG_CAT(ppc_launchers_NP, DG_NP) = {launch_update, launch_update_energy, kTile,
                                                              "pair-per-cell, circulant shared-memory tile, sorted chunks"};
 
 }  // namespace dg

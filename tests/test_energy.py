@@ -85,12 +85,13 @@ def test_heating_n1_closed_form(oracle):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("ncells", [1501, 2048, 2570])
-@pytest.mark.parametrize("N", [1, 2, 4, 7, 8, 12, 13, 16])
+@pytest.mark.parametrize("N", [1, 2, 4, 7, 8, 12, 13, 14, 15, 16])
 def test_gpu_energy_update_matches_the_oracle(dg, oracle, cuda, N, ncells):
     """dg_drag_update_energy through the C ABI against the oracle: momenta at BASELINE.json's tolerance, gas energy to
     1e-13 of the cell's energy scale (E_g and the kinetic energies: a handful of fp64 products and one difference).
-    N <= 12 is one launch of the sorted-tile kernel (whole tiles by bulk copies for the even cell counts, per-thread copies
-    for the odd one and the ragged tails), N >= 13 three launches."""
+    One launch for every N: the sorted-tile kernel for N <= 12 (whole tiles by bulk copies for the even cell counts,
+    per-thread copies for the odd one and the ragged tails), the pair-per-cell kernel for N >= 13 (each lane sums over the
+    rows it applies; the ragged last chunk has lanes without a cell)."""
     from paper_2509_25347_b200 import workloads as W
     wl = W.make_workload(5, ncells=ncells, N=N, device=cuda)
     wl.rho_d[0, ::5] = 0.0
