@@ -388,6 +388,45 @@ def test_extreme_stiffness_against_mpmath(dg, cuda, N):
                     assert abs(mpf(float(o[comp, k])) - refs[comp][k]) <= PARITY_TOL * scale, (N, c, v, comp, k)
 
 
+@pytest.mark.parametrize("N", [4, 12, 13, 16])
+def test_extreme_stiffness_against_mpmath_across_tiles(dg, cuda, N):
+    """The same arbitrary-precision referee as above (mpmath.expm at 90 digits on Eq. 17 retyped here), but on an array
+    of several hundred tiles — two per block of the persistent pair-per-cell kernel — with the ~1e10-norm cells
+    scattered through it instead of sitting in the first tile: in every tile they share chunks, and a chunk's common
+    (m, s), with cells of ordinary stiffness.  Default kernels of both families at their smallest and largest N."""
+    import mpmath as mpm
+    from mpmath import mp, mpf
+    mp.dps = 90
+    sms = torch.cuda.get_device_properties(cuda).multi_processor_count
+    ncells = 128 * sms * 2 + 91
+    wl = _extreme_workload(N, cuda, ncells=ncells)
+    stiff = torch.arange(37, ncells, 4099, device=cuda)          # 10 cells, far apart, off every tile boundary
+    wl.t_s[:, stiff] = 1e-12
+    out, s, m = dg.dg_drag_update_ex(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all())
+    assert int(s[stiff].min()) >= 30
+    drift = (out.sum(dim=1) - wl.p_in.sum(dim=1)).abs() / wl.p_in.abs().sum(dim=1)
+    assert float(drift.max()) <= CONS_TOL
+    # the scattered stiff cells, their right-hand neighbours (ordinary cells that may share their chunk), the last cell
+    check = torch.unique(torch.cat([stiff[::2].cpu(), stiff[1::3].cpu() + 1, torch.tensor([ncells - 1])]))
+    rho_g, rho_d, t_s, p_in = wl.cells(check)
+    got = out[:, :, check.to(cuda)].cpu().numpy()
+    n = N + 1
+    for j in range(len(check)):
+        A = mpm.zeros(n, n)
+        for i in range(N):
+            alpha = mpf(wl.dt) / mpf(float(t_s[i, j]))
+            e = mpf(float(rho_d[i, j])) / mpf(float(rho_g[j]))
+            A[0, 0] -= e * alpha; A[0, i + 1] = alpha; A[i + 1, 0] = e * alpha; A[i + 1, i + 1] = -alpha
+        E = mpm.expm(A, method="taylor")
+        scale = max(abs(float(x)) for x in p_in[:, :, j].ravel())
+        for comp in range(3):
+            ref = E * mpm.matrix([mpf(float(x)) for x in p_in[comp, :, j]])
+            for k in range(n):
+                assert abs(mpf(float(got[comp, k, j])) - ref[k]) <= PARITY_TOL * scale, (N, int(check[j]), comp, k)
+
+
 @pytest.mark.parametrize("N,variant", [(14, 0), (16, 0), (16, 2), (4, 2), (8, 2), (8, 1), (3, 0), (13, 0), (16, 4), (7, 4),
                                        (1, 7), (2, 0), (8, 7), (12, 0)])
 @pytest.mark.parametrize("ncells", [512, 515, 2050])
