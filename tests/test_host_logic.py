@@ -65,8 +65,11 @@ def test_argument_validation_without_a_gpu(dg):
     for N in range(1, 17):   # the default mapping named for every N: sorted tiles up to 12, pair per cell above
         name = dg.dg_variant_name(N)
         assert ("thread-per-cell" in name) == (N <= 12) and ("pair-per-cell" in name) == (N >= 13), (N, name)
-    for st in range(6):
+    for st in range(7):
         assert dg.raw().dg_status_string(st).decode().startswith("DG_")
+    # the test hook that replaced the DG_HOST_MAX_PITCH environment variable
+    assert lib.dg_host_set_max_pitch(-1) == dg.DG_EINVAL
+    assert lib.dg_host_set_max_pitch(4096) == dg.DG_OK and lib.dg_host_set_max_pitch(0) == dg.DG_OK
     with pytest.raises(TypeError):
         dg.dg_drag_update(torch.zeros(4), torch.zeros(1, 4), torch.zeros(1, 4), 0.1, torch.zeros(3, 2, 4))
 
