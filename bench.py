@@ -379,19 +379,15 @@ def _timed_ms(f, steps, warmup):
 
 
 def bench_energy(dg, wl, p_out, ms_update, hbm_gbs, steps=5, warmup=2):
-    """dg_drag_update_energy (Eq. 4, R20).  N <= 12: ONE launch of the sorted-tile kernel,
-    which forms the kinetic-energy sums from the tile it holds anyway — algorithmic bytes per cell 8(8N+7) + 16 (E read
-    and written).  N >= 13: the fused update between two O(N) kernels that read the densities and the momenta before /
-    after it — the update's 8(8N+7) plus 8(2(1 + N + 3n) + 3) bytes per cell."""
+    """dg_drag_update_energy (Eq. 4, R20): ONE launch of the default kernel for N, which
+    forms the kinetic-energy sums from the values its apply step holds anyway — algorithmic bytes per cell 8(8N+7) + 16
+    (E read and written)."""
     E_in = torch.ones(wl.ncells, dtype=torch.float64, device=wl.rho_g.device)
     E_out = torch.empty_like(E_in)
     ms = _timed_ms(lambda: dg.dg_drag_update_energy(wl.rho_g, wl.rho_d, wl.t_s, wl.dt, wl.p_in, E_in, 0.5, p_out=p_out,
                                                     E_out=E_out), steps, warmup)
-    n = wl.N + 1
-    fused = wl.N <= 12
-    extra = 16 if fused else 8 * (2 * (1 + wl.N + 3 * n) + 3)
-    total = algorithmic_bytes_per_cell(wl.N) + extra
-    return {"ms_per_launch_sequence": ms, "launches": 1 if fused else 3, "cells_per_s": wl.ncells / (ms * 1e-3),
+    total = algorithmic_bytes_per_cell(wl.N) + 16
+    return {"ms_per_launch_sequence": ms, "launches": 1, "cells_per_s": wl.ncells / (ms * 1e-3),
             "over_plain_update": ms / ms_update, "algorithmic_bytes_per_cell": total,
             "hbm_frac": total * wl.ncells / (ms * 1e-3) / 1e9 / hbm_gbs}
 
